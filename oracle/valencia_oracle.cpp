@@ -1,0 +1,674 @@
+// valencia_oracle.cpp -- CPU ORACLE for the FP64 Valencia GRMHD right-hand side.
+//
+// THIS FILE IS TEST INFRASTRUCTURE.  It is the plain, slow, obviously-correct statement of what
+// the hot path computes, written from the paper (GRaM-X, arxiv 2210.17509; citations are
+// PAPER.md line numbers + equation) and from the readings R1..R29 listed in DESIGN.md.  Only
+// tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call
+// it.  It shares no code, header, table or constant generator with the CUDA path
+// (paper_2210_17509_b200/csrc) and neither includes the other.
+//
+// Parity pins: every exported function below is pinned by tests/test_oracle_pins*.py against
+// closed forms, invariants and the paper's printed Balsara-1 values (tests/golden/).  Conventions
+// that no external value can pin -- WENO_EPS, V2MAX, the fast-speed approximation a^2 (R8) and
+// the MC limiter -- are listed as "parity unpinned (convention)" in DESIGN.md.
+//
+// No blocking, fusion or re-ordering beyond what the algorithm states: per direction, per grid
+// line: reconstruct (O2) -> face metric (O1) -> admissibility (O3) -> state (O4) -> flux (O5)
+// -> wave speeds (O6) -> HLLE (O7) -> divergence; then derivatives (O8) and sources (O9).
+//
+// The whole algorithm is templated on the scalar type `R`:
+//   double       -- THE oracle
+//   long double  -- adjudicator (quantifies the oracle's own rounding, pin P18)
+//   Counted      -- a double that counts its operations (official algorithmic flop count)
+//
+// Build: g++ -O2 -fopenmp -ffp-contract=off -fno-fast-math -shared -fPIC (see oracle/build.py).
+
+#include <cmath>
+#include <cstddef>
+#include <cstring>
+#include <type_traits>
+#include <vector>
+
+namespace {
+
+// ---- conventions (R4, R5): compile-time constants -------------------------------------------
+constexpr double WENO_EPS = 1e-26;       // R4: Jiang-Shu epsilon
+constexpr double V2MAX    = 1.0 - 1e-4;  // R5: admissibility bound on v^2 (W_max = 100)
+
+enum { RECON_MINMOD = 0, RECON_MC = 1, RECON_WENO5 = 2 };
+
+// symmetric 3x3 storage: xx xy xz yy yz zz
+constexpr int SYM[3][3] = {{0, 1, 2}, {1, 3, 4}, {2, 4, 5}};
+
+// ---- operation-counting scalar ----------------------------------------------------------------
+struct OpCount { unsigned long long add, mul, div, sqrt; };
+thread_local OpCount t_ops = {0, 0, 0, 0};
+
+struct Counted {
+    double v;
+    Counted() : v(0.0) {}
+    Counted(double x) : v(x) {}
+};
+inline Counted operator+(Counted a, Counted b) { ++t_ops.add; return Counted(a.v + b.v); }
+inline Counted operator-(Counted a, Counted b) { ++t_ops.add; return Counted(a.v - b.v); }
+inline Counted operator*(Counted a, Counted b) { ++t_ops.mul; return Counted(a.v * b.v); }
+inline Counted operator/(Counted a, Counted b) { ++t_ops.div; return Counted(a.v / b.v); }
+inline Counted operator-(Counted a) { return Counted(-a.v); }   // sign flip: free
+inline Counted& operator+=(Counted& a, Counted b) { a = a + b; return a; }
+inline Counted& operator-=(Counted& a, Counted b) { a = a - b; return a; }
+inline bool operator>(Counted a, Counted b) { return a.v > b.v; }
+inline bool operator<(Counted a, Counted b) { return a.v < b.v; }
+inline bool operator<=(Counted a, Counted b) { return a.v <= b.v; }
+inline bool operator>=(Counted a, Counted b) { return a.v >= b.v; }
+
+inline double      o_sqrt(double x) { return std::sqrt(x); }
+inline long double o_sqrt(long double x) { return sqrtl(x); }
+inline Counted     o_sqrt(Counted x) { ++t_ops.sqrt; return Counted(std::sqrt(x.v)); }
+inline double      o_abs(double x) { return std::fabs(x); }
+inline long double o_abs(long double x) { return fabsl(x); }
+inline Counted     o_abs(Counted x) { return Counted(std::fabs(x.v)); }
+inline double      to_double(double x) { return x; }
+inline double      to_double(long double x) { return (double)x; }
+inline double      to_double(Counted x) { return x.v; }
+
+template <class R> inline R o_min(R a, R b) { return (b < a) ? b : a; }
+template <class R> inline R o_max(R a, R b) { return (b > a) ? b : a; }
+
+// ---- O2: reconstruction of one cell (refs [31],[32]) ---------------------
+// Input: the five cell values (a,b,c,d,e) = (q_{i-2}, q_{i-1}, q_i, q_{i+1}, q_{i+2}).
+// Output: qm = value at face i-1/2 taken from cell i;  qp = value at face i+1/2 taken from cell i.
+
+// TVD, minmod slope (l.255 "TVD reconstruction with the minmod limiter"; R3)
+template <class R> void recon_minmod(R b, R c, R d, R& qm, R& qp) {
+    R dm = c - b, dp = d - c;
+    R sigma = R(0.0);
+    if (dm * dp > R(0.0)) {
+        R m = o_min(o_abs(dm), o_abs(dp));
+        sigma = (dm > R(0.0)) ? m : -m;
+    }
+    qm = c - R(0.5) * sigma;
+    qp = c + R(0.5) * sigma;
+}
+
+// TVD, monotonised-central slope (north_star only; R3)
+template <class R> void recon_mc(R b, R c, R d, R& qm, R& qp) {
+    R dm = c - b, dp = d - c;
+    R sigma = R(0.0);
+    if (dm * dp > R(0.0)) {
+        R m = o_min(o_min(R(2.0) * o_abs(dm), R(2.0) * o_abs(dp)), R(0.5) * o_abs(dm + dp));
+        sigma = (dm > R(0.0)) ? m : -m;
+    }
+    qm = c - R(0.5) * sigma;
+    qp = c + R(0.5) * sigma;
+}
+
+// WENO5, Jiang-Shu (ref [32] = Shu 1998; R4).  The three smoothness indicators belong to the cell
+// and are shared by its two faces (the mirrored stencil has beta0 <-> beta2).
+template <class R> R weno5_combine(R p0, R p1, R p2, R b0, R b1, R b2) {
+    R e0 = R(WENO_EPS) + b0, e1 = R(WENO_EPS) + b1, e2 = R(WENO_EPS) + b2;
+    R a0 = R(0.1) / (e0 * e0);
+    R a1 = R(0.6) / (e1 * e1);
+    R a2 = R(0.3) / (e2 * e2);
+    return (a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2);
+}
+template <class R> void recon_weno5(R a, R b, R c, R d, R e, R& qm, R& qp) {
+    R t;
+    t = a - R(2.0) * b + c;              R b0 = R(13.0 / 12.0) * t * t;
+    t = a - R(4.0) * b + R(3.0) * c;     b0 = b0 + R(0.25) * t * t;
+    t = b - R(2.0) * c + d;              R b1 = R(13.0 / 12.0) * t * t;
+    t = b - d;                           b1 = b1 + R(0.25) * t * t;
+    t = c - R(2.0) * d + e;              R b2 = R(13.0 / 12.0) * t * t;
+    t = R(3.0) * c - R(4.0) * d + e;     b2 = b2 + R(0.25) * t * t;
+    // q^+_i : stencil (a,b,c,d,e)
+    R p0 = (R(2.0) * a - R(7.0) * b + R(11.0) * c) / R(6.0);
+    R p1 = (-b + R(5.0) * c + R(2.0) * d) / R(6.0);
+    R p2 = (R(2.0) * c + R(5.0) * d - e) / R(6.0);
+    qp = weno5_combine(p0, p1, p2, b0, b1, b2);
+    // q^-_i : same formula on the mirrored stencil (e,d,c,b,a); its indicators are (b2,b1,b0)
+    R m0 = (R(2.0) * e - R(7.0) * d + R(11.0) * c) / R(6.0);
+    R m1 = (-d + R(5.0) * c + R(2.0) * b) / R(6.0);
+    R m2 = (R(2.0) * c + R(5.0) * b - a) / R(6.0);
+    qm = weno5_combine(m0, m1, m2, b2, b1, b0);
+}
+template <class R> void recon_cell(int recon, R a, R b, R c, R d, R e, R& qm, R& qp) {
+    if (recon == RECON_WENO5) recon_weno5(a, b, c, d, e, qm, qp);
+    else if (recon == RECON_MC) recon_mc(b, c, d, qm, qp);
+    else recon_minmod(b, c, d, qm, qp);
+}
+
+// ---- metric at a point (face or centre) -----------------------------------------------------------
+template <class R> struct Metric {
+    R alp, beta[3], g[6];   // lapse, shift beta^i, gamma_ij
+    R det, sqrtg;           // det(gamma_ij), sqrt of it
+    R gu[6];                // inverse gamma^{ij}
+};
+// determinant by cofactor expansion, inverse = cofactor/det (O1)
+template <class R> void metric_complete(Metric<R>& m) {
+    const R gxx = m.g[0], gxy = m.g[1], gxz = m.g[2], gyy = m.g[3], gyz = m.g[4], gzz = m.g[5];
+    R cxx = gyy * gzz - gyz * gyz;
+    R cxy = gxz * gyz - gxy * gzz;
+    R cxz = gxy * gyz - gxz * gyy;
+    R cyy = gxx * gzz - gxz * gxz;
+    R cyz = gxy * gxz - gxx * gyz;
+    R czz = gxx * gyy - gxy * gxy;
+    m.det = gxx * cxx + gxy * cxy + gxz * cxz;
+    m.sqrtg = o_sqrt(m.det);
+    m.gu[0] = cxx / m.det; m.gu[1] = cxy / m.det; m.gu[2] = cxz / m.det;
+    m.gu[3] = cyy / m.det; m.gu[4] = cyz / m.det; m.gu[5] = czz / m.det;
+}
+// face metric along d needs only det, sqrt(gamma) and gamma^{dd} (O1)
+template <class R> void metric_complete_face(Metric<R>& m, int d) {
+    const R gxx = m.g[0], gxy = m.g[1], gxz = m.g[2], gyy = m.g[3], gyz = m.g[4], gzz = m.g[5];
+    R cxx = gyy * gzz - gyz * gyz;
+    R cxy = gxz * gyz - gxy * gzz;
+    R cxz = gxy * gyz - gxz * gyy;
+    m.det = gxx * cxx + gxy * cxy + gxz * cxz;
+    m.sqrtg = o_sqrt(m.det);
+    R cdd = (d == 0) ? cxx : (d == 1) ? gxx * gzz - gxz * gxz : gxx * gyy - gxy * gxy;
+    m.gu[SYM[d][d]] = cdd / m.det;
+}
+template <class R> inline R lower(const Metric<R>& m, const R v[3], int i) {
+    return m.g[SYM[i][0]] * v[0] + m.g[SYM[i][1]] * v[1] + m.g[SYM[i][2]] * v[2];
+}
+
+// ---- O3: admissibility of a reconstructed state (R5).  Written so NaN fails it. ---------------------
+template <class R> bool admissible(const R P[8], const Metric<R>& m) {
+    const R v[3] = {P[1], P[2], P[3]};
+    R v2 = lower(m, v, 0) * v[0] + lower(m, v, 1) * v[1] + lower(m, v, 2) * v[2];
+    return (P[0] > R(0.0)) && (P[4] > R(0.0)) && (v2 < R(V2MAX));
+}
+
+// ---- O4: primitive -> conserved, Eqs. (6)-(10) ------------------------------------
+// Also returns the scalars the flux, the wave speeds and the sources reuse.
+template <class R> struct State {
+    R vl[3], v2, W, Bl[3], B2, Bv, ab0, b2, bl[3], p, rhoh, rhohs, Ps;
+    R U[8];   // D, S_x, S_y, S_z, tau, calB^x, calB^y, calB^z
+};
+template <class R> void prim2con_point(const R P[8], const Metric<R>& m, R gamma, State<R>& s) {
+    const R rho = P[0], eps = P[4];
+    const R v[3] = {P[1], P[2], P[3]};
+    const R B[3] = {P[5], P[6], P[7]};
+    for (int i = 0; i < 3; ++i) s.vl[i] = lower(m, v, i);                     // v_i = gamma_ij v^j
+    s.v2 = s.vl[0] * v[0] + s.vl[1] * v[1] + s.vl[2] * v[2];
+    s.W = R(1.0) / o_sqrt(R(1.0) - s.v2);                                      // l.98
+    for (int i = 0; i < 3; ++i) s.Bl[i] = lower(m, B, i);
+    s.B2 = s.Bl[0] * B[0] + s.Bl[1] * B[1] + s.Bl[2] * B[2];
+    s.Bv = s.Bl[0] * v[0] + s.Bl[1] * v[1] + s.Bl[2] * v[2];
+    s.ab0 = s.W * s.Bv;                                                        // alpha b^0
+    s.b2 = s.B2 / (s.W * s.W) + s.Bv * s.Bv;                                   // b^2
+    for (int i = 0; i < 3; ++i) s.bl[i] = s.Bl[i] / s.W + s.ab0 * s.vl[i];     // b_i
+    s.p = (gamma - R(1.0)) * rho * eps;                                        // l.138 Gamma-law
+    s.rhoh = rho * (R(1.0) + eps) + s.p;                                       // rho h
+    s.rhohs = s.rhoh + s.b2;                                                   // rho h*   (Eq. 5)
+    s.Ps = s.p + R(0.5) * s.b2;                                                // P*
+    const R W2 = s.W * s.W;
+    s.U[0] = m.sqrtg * rho * s.W;                                              // Eq. (6)
+    for (int j = 0; j < 3; ++j)
+        s.U[1 + j] = m.sqrtg * (s.rhohs * W2 * s.vl[j] - s.ab0 * s.bl[j]);     // Eq. (7)
+    s.U[4] = m.sqrtg * (s.rhohs * W2 - s.Ps - s.ab0 * s.ab0) - s.U[0];         // Eq. (8)
+    for (int k = 0; k < 3; ++k) s.U[5 + k] = m.sqrtg * B[k];                   // Eq. (9)
+}
+
+// ---- O5: physical flux along d, Eq. (12) (l.108), vtilde^i = v^i - beta^i/alpha (l.114) -----------------
+template <class R> void flux_point(const R P[8], const Metric<R>& m, const State<R>& s, int d, R F[8]) {
+    const R v[3] = {P[1], P[2], P[3]};
+    R vt[3];
+    for (int i = 0; i < 3; ++i) vt[i] = v[i] - m.beta[i] / m.alp;
+    const R sgPs = m.sqrtg * s.Ps;
+    const R Bd_W = s.U[5 + d] / s.W;                                           // calB^d / W
+    F[0] = m.alp * (s.U[0] * vt[d]);
+    for (int j = 0; j < 3; ++j) {
+        R t = s.U[1 + j] * vt[d] - s.bl[j] * Bd_W;
+        if (j == d) t = t + sgPs;
+        F[1 + j] = m.alp * t;
+    }
+    F[4] = m.alp * (s.U[4] * vt[d] + sgPs * v[d] - s.ab0 * Bd_W);
+    for (int k = 0; k < 3; ++k) F[5 + k] = m.alp * (s.U[5 + k] * vt[d] - s.U[5 + d] * vt[k]);
+}
+
+// ---- O6: fast-magnetosonic characteristic speeds along d (R8) ------------------------------------------
+template <class R>
+void wavespeeds_point(const R P[8], const Metric<R>& m, const State<R>& s, int d, R gamma, R& lam_m, R& lam_p) {
+    const R vd = P[1 + d];
+    R cs2 = gamma * s.p / s.rhoh;
+    R va2 = s.b2 / s.rhohs;
+    R a2 = cs2 + va2 - cs2 * va2;
+    R one_v2a2 = R(1.0) - s.v2 * a2;
+    R disc = a2 * (R(1.0) - s.v2) * (m.gu[SYM[d][d]] * one_v2a2 - vd * vd * (R(1.0) - a2));
+    if (!(disc > R(0.0))) disc = R(0.0);
+    R root = o_sqrt(disc);
+    lam_p = m.alp * (vd * (R(1.0) - a2) + root) / one_v2a2 - m.beta[d];
+    lam_m = m.alp * (vd * (R(1.0) - a2) - root) / one_v2a2 - m.beta[d];
+}
+
+// ---- O7: HLLE flux (refs [33-35]; R9) -----------------------------------------------------------------------
+template <class R>
+void hlle(const R UL[8], const R FL[8], R lmL, R lpL, const R UR[8], const R FR[8], R lmR, R lpR, R Fh[8]) {
+    R lm = o_min(R(0.0), o_min(lmL, lmR));
+    R lp = o_max(R(0.0), o_max(lpL, lpR));
+    for (int c = 0; c < 8; ++c)
+        Fh[c] = (lp * FL[c] - lm * FR[c] + lp * lm * (UR[c] - UL[c])) / (lp - lm);
+}
+
+// One interface: metric already averaged to the face (alp, beta, g filled), reconstructed left and
+// right primitive states PL/PR and the centre values CL/CR of their donor cells (O3 fallback).
+template <class R>
+void face_flux(Metric<R>& mf, int d, R gamma, const R PLin[8], const R PRin[8], const R CL[8], const R CR[8],
+               R Fh[8], unsigned long long* nfallback) {
+    metric_complete_face(mf, d);
+    R PL[8], PR[8];
+    bool okL = admissible(PLin, mf), okR = admissible(PRin, mf);
+    for (int q = 0; q < 8; ++q) { PL[q] = okL ? PLin[q] : CL[q]; PR[q] = okR ? PRin[q] : CR[q]; }
+    if (nfallback) *nfallback += (okL ? 0 : 1) + (okR ? 0 : 1);
+    State<R> sL, sR;
+    R FL[8], FR[8], lmL, lpL, lmR, lpR;
+    prim2con_point(PL, mf, gamma, sL); flux_point(PL, mf, sL, d, FL); wavespeeds_point(PL, mf, sL, d, gamma, lmL, lpL);
+    prim2con_point(PR, mf, gamma, sR); flux_point(PR, mf, sR, d, FR); wavespeeds_point(PR, mf, sR, d, gamma, lmR, lpR);
+    hlle(sL.U, FL, lmL, lpL, sR.U, FR, lmR, lpR, Fh);
+}
+
+// ---- O9: geometric sources at a cell centre, Eq. (13) (l.112) in 3+1 form (R12-R14) -------------------
+// dm[j][f] = d/dx^j of metric field f (f: alp, betax, betay, betaz, gxx, gxy, gxz, gyy, gyz, gzz).
+template <class R>
+void sources_point(const R P[8], Metric<R>& m, const R K[6], const R dm[3][10], R gamma, R S[8]) {
+    metric_complete(m);
+    State<R> s;
+    prim2con_point(P, m, gamma, s);
+    const R v[3] = {P[1], P[2], P[3]};
+    const R B[3] = {P[5], P[6], P[7]};
+    const R alp = m.alp;
+    const R W2 = s.W * s.W;
+    R vt[3], bu[3];
+    for (int i = 0; i < 3; ++i) vt[i] = v[i] - m.beta[i] / alp;
+    for (int i = 0; i < 3; ++i) bu[i] = B[i] / s.W + s.ab0 * vt[i];            // b^i
+    // stress-energy tensor, Eq. (5) with u^0 = W/alpha, u^i = W vtilde^i, g^{mu nu} of the 3+1 split
+    R T00 = (s.rhohs * W2 - s.Ps - s.ab0 * s.ab0) / (alp * alp);
+    R T0[3], T[3][3], T0l[3], betal[3];
+    for (int i = 0; i < 3; ++i)
+        T0[i] = s.rhohs * W2 * vt[i] / alp + s.Ps * m.beta[i] / (alp * alp) - s.ab0 * bu[i] / alp;
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j)
+            T[i][j] = s.rhohs * W2 * vt[i] * vt[j] + s.Ps * (m.gu[SYM[i][j]] - m.beta[i] * m.beta[j] / (alp * alp)) -
+                      bu[i] * bu[j];
+    for (int k = 0; k < 3; ++k) betal[k] = lower(m, m.beta, k);
+    for (int k = 0; k < 3; ++k)
+        T0l[k] = betal[k] * T00 + m.g[SYM[k][0]] * T0[0] + m.g[SYM[k][1]] * T0[1] + m.g[SYM[k][2]] * T0[2];
+    for (int c = 0; c < 8; ++c) S[c] = R(0.0);
+    const R pref = alp * m.sqrtg;
+    // momentum sources
+    for (int j = 0; j < 3; ++j) {
+        const R da = dm[j][0];
+        R bbdg = R(0.0), t0bdg = R(0.0), tdg = R(0.0), t0ldb = R(0.0);
+        for (int k = 0; k < 3; ++k)
+            for (int l = 0; l < 3; ++l) {
+                const R dg = dm[j][4 + SYM[k][l]];
+                bbdg = bbdg + m.beta[k] * m.beta[l] * dg;
+                t0bdg = t0bdg + T0[k] * m.beta[l] * dg;
+                tdg = tdg + T[k][l] * dg;
+            }
+        for (int k = 0; k < 3; ++k) t0ldb = t0ldb + T0l[k] * dm[j][1 + k];
+        S[1 + j] = pref * (T00 * (R(0.5) * bbdg - alp * da) + t0bdg + t0ldb + R(0.5) * tdg);
+    }
+    // energy source
+    R bbK = R(0.0), tK = R(0.0), bda = R(0.0), t0term = R(0.0);
+    for (int i = 0; i < 3; ++i) {
+        R bK = R(0.0);
+        for (int j = 0; j < 3; ++j) {
+            bbK = bbK + m.beta[i] * m.beta[j] * K[SYM[i][j]];
+            tK = tK + T[i][j] * K[SYM[i][j]];
+            bK = bK + m.beta[j] * K[SYM[i][j]];
+        }
+        bda = bda + m.beta[i] * dm[i][0];
+        t0term = t0term + T0[i] * (R(2.0) * bK - dm[i][0]);
+    }
+    S[4] = pref * (T00 * (bbK - bda) + t0term + tK);
+}
+
+// ---- whole right-hand side of one box ------------------------------------------------------------------------
+struct Grid {
+    int n[3], g, N[3];
+    size_t ncell;
+    size_t idx(int i, int j, int k) const {
+        return (size_t)(i + g) + (size_t)N[0] * ((size_t)(j + g) + (size_t)N[1] * (size_t)(k + g));
+    }
+};
+
+template <class R>
+void rhs_box(const Grid& G, const double* prim, const double* met, const double* Kc, const double dx[3], int recon,
+             double gamma_d, double* out, unsigned long long* fallback_total) {
+    const R gamma = R(gamma_d);
+    const size_t NC = G.ncell;
+    unsigned long long nfb_all = 0;
+    OpCount ops_all = {0, 0, 0, 0};
+
+    // accumulator in the working precision R (for R = double it is `out` itself); interior cells start
+    // from zero; ghost cells of `out` are never touched (R23)
+    std::vector<R> acc_store;
+    R* acc;
+    if constexpr (std::is_same<R, double>::value) {
+        acc = out;
+    } else {
+        acc_store.assign(8 * NC, R(0.0));
+        acc = acc_store.data();
+    }
+    for (int c = 0; c < 8; ++c)
+        for (int k = 0; k < G.n[2]; ++k)
+            for (int j = 0; j < G.n[1]; ++j)
+                for (int i = 0; i < G.n[0]; ++i) acc[c * NC + G.idx(i, j, k)] = R(0.0);
+
+    // per direction: lines along d
+    for (int d = 0; d < 3; ++d) {
+        const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+        const int nd = G.n[d];
+        const long nlines = (long)G.n[d1] * G.n[d2];
+#pragma omp parallel
+        {
+            unsigned long long nfb = 0;
+            std::vector<R> qm(8 * (size_t)(nd + 2)), qp(8 * (size_t)(nd + 2)), Fh(8 * (size_t)(nd + 1));
+#pragma omp for schedule(static)
+            for (long line = 0; line < nlines; ++line) {
+                int ijk[3];
+                ijk[d1] = (int)(line % G.n[d1]);
+                ijk[d2] = (int)(line / G.n[d1]);
+                auto at = [&](int s) {   // index of cell s along the line
+                    int c3[3] = {ijk[0], ijk[1], ijk[2]};
+                    c3[d] = s;
+                    return G.idx(c3[0], c3[1], c3[2]);
+                };
+                // O2: reconstruct cells -1 .. nd
+                for (int s = -1; s <= nd; ++s)
+                    for (int q = 0; q < 8; ++q) {
+                        const double* f = prim + q * NC;
+                        R a = (recon == RECON_WENO5) ? R(f[at(s - 2)]) : R(0.0);
+                        R e = (recon == RECON_WENO5) ? R(f[at(s + 2)]) : R(0.0);
+                        recon_cell<R>(recon, a, R(f[at(s - 1)]), R(f[at(s)]), R(f[at(s + 1)]), e,
+                                      qm[q * (nd + 2) + s + 1], qp[q * (nd + 2) + s + 1]);
+                    }
+                // faces f = 0 .. nd between cells f-1 and f
+                for (int f = 0; f <= nd; ++f) {
+                    const size_t iL = at(f - 1), iR = at(f);
+                    Metric<R> mf;
+                    mf.alp = R(0.5) * (R(met[0 * NC + iL]) + R(met[0 * NC + iR]));                       // O1
+                    for (int i = 0; i < 3; ++i)
+                        mf.beta[i] = R(0.5) * (R(met[(1 + i) * NC + iL]) + R(met[(1 + i) * NC + iR]));
+                    for (int c = 0; c < 6; ++c)
+                        mf.g[c] = R(0.5) * (R(met[(4 + c) * NC + iL]) + R(met[(4 + c) * NC + iR]));
+                    R PL[8], PR[8], CL[8], CR[8];
+                    for (int q = 0; q < 8; ++q) {
+                        PL[q] = qp[q * (nd + 2) + f];       // q^+ of cell f-1
+                        PR[q] = qm[q * (nd + 2) + f + 1];   // q^- of cell f
+                        CL[q] = R(prim[q * NC + iL]);
+                        CR[q] = R(prim[q * NC + iR]);
+                    }
+                    face_flux(mf, d, gamma, PL, PR, CL, CR, &Fh[8 * (size_t)f], &nfb);
+                }
+                // O7: out -= (F_{f+1} - F_f)/dx_d
+                for (int s = 0; s < nd; ++s)
+                    for (int c = 0; c < 8; ++c) {
+                        R div = (Fh[8 * (size_t)(s + 1) + c] - Fh[8 * (size_t)s + c]) / R(dx[d]);
+                        acc[c * NC + at(s)] -= div;
+                    }
+            }
+#pragma omp critical
+            {
+                nfb_all += nfb;
+                ops_all.add += t_ops.add; ops_all.mul += t_ops.mul; ops_all.div += t_ops.div; ops_all.sqrt += t_ops.sqrt;
+                t_ops = {0, 0, 0, 0};
+            }
+        }
+    }
+
+    // O8 + O9: sources
+#pragma omp parallel
+    {
+#pragma omp for schedule(static) collapse(2)
+        for (int k = 0; k < G.n[2]; ++k)
+            for (int j = 0; j < G.n[1]; ++j)
+                for (int i = 0; i < G.n[0]; ++i) {
+                    const size_t c0 = G.idx(i, j, k);
+                    const size_t stride[3] = {1, (size_t)G.N[0], (size_t)G.N[0] * G.N[1]};
+                    R dm[3][10];
+                    for (int a = 0; a < 3; ++a)
+                        for (int f = 0; f < 10; ++f) {
+                            const double* m = met + f * NC + c0;
+                            const long s = (long)stride[a];
+                            // O8: grouped so that a constant field differentiates to exactly zero
+                            dm[a][f] = (R(8.0) * (R(m[s]) - R(m[-s])) - (R(m[2 * s]) - R(m[-2 * s]))) / (R(12.0) * R(dx[a]));
+                        }
+                    Metric<R> mc;
+                    mc.alp = R(met[c0]);
+                    for (int a = 0; a < 3; ++a) mc.beta[a] = R(met[(1 + a) * NC + c0]);
+                    for (int c = 0; c < 6; ++c) mc.g[c] = R(met[(4 + c) * NC + c0]);
+                    R P[8], K[6], S[8];
+                    for (int q = 0; q < 8; ++q) P[q] = R(prim[q * NC + c0]);
+                    for (int c = 0; c < 6; ++c) K[c] = R(Kc[c * NC + c0]);
+                    sources_point(P, mc, K, dm, gamma, S);
+                    for (int c = 1; c <= 4; ++c) acc[c * NC + c0] += S[c];
+                }
+#pragma omp critical
+        {
+            ops_all.add += t_ops.add; ops_all.mul += t_ops.mul; ops_all.div += t_ops.div; ops_all.sqrt += t_ops.sqrt;
+            t_ops = {0, 0, 0, 0};
+        }
+    }
+    if constexpr (!std::is_same<R, double>::value) {
+        for (int c = 0; c < 8; ++c)
+            for (int k = 0; k < G.n[2]; ++k)
+                for (int j = 0; j < G.n[1]; ++j)
+                    for (int i = 0; i < G.n[0]; ++i) out[c * NC + G.idx(i, j, k)] = to_double(acc[c * NC + G.idx(i, j, k)]);
+    }
+    if (fallback_total) *fallback_total += nfb_all;
+    t_ops = ops_all;   // left for the caller (counting instance only)
+}
+
+template <class R>
+int rhs_all(const int n[3], int nbox, const double* prim, const double* met, const double* K, const double dx[3],
+            int g, int recon, double gamma, double* out, unsigned long long* nfallback, OpCount* ops) {
+    if (!n || !prim || !met || !K || !dx || !out) return 1;
+    if (n[0] < 1 || n[1] < 1 || n[2] < 1 || nbox < 1) return 1;
+    if (recon != RECON_MINMOD && recon != RECON_MC && recon != RECON_WENO5) return 1;
+    if (g < (recon == RECON_WENO5 ? 3 : 2)) return 1;   // R29
+    if (!(gamma > 1.0) || !(dx[0] > 0.0) || !(dx[1] > 0.0) || !(dx[2] > 0.0)) return 1;
+    Grid G;
+    for (int a = 0; a < 3; ++a) { G.n[a] = n[a]; G.N[a] = n[a] + 2 * g; }
+    G.g = g;
+    G.ncell = (size_t)G.N[0] * G.N[1] * G.N[2];
+    unsigned long long nfb = 0;
+    OpCount tot = {0, 0, 0, 0};
+    for (int b = 0; b < nbox; ++b) {
+        t_ops = {0, 0, 0, 0};
+        rhs_box<R>(G, prim + (size_t)b * 8 * G.ncell, met + (size_t)b * 10 * G.ncell, K + (size_t)b * 6 * G.ncell, dx,
+                   recon, gamma, out + (size_t)b * 8 * G.ncell, &nfb);
+        tot.add += t_ops.add; tot.mul += t_ops.mul; tot.div += t_ops.div; tot.sqrt += t_ops.sqrt;
+    }
+    if (nfallback) *nfallback = nfb;
+    if (ops) *ops = tot;
+    return 0;
+}
+
+// ---- support code for the short Balsara-1 evolution (R21, R22): ideal-gas con2prim -----------------------
+// 1-D Newton/bisection solve in z = rho h W^2 on the undensitised conserved variables.
+int con2prim_point(const double U[8], const Metric<double>& m, double gamma, double P[8]) {
+    const double sg = m.sqrtg;
+    const double D = U[0] / sg, tau = U[4] / sg;
+    const double Sl[3] = {U[1] / sg, U[2] / sg, U[3] / sg};
+    const double B[3] = {U[5] / sg, U[6] / sg, U[7] / sg};
+    double Su[3], Bl[3];
+    for (int i = 0; i < 3; ++i) {
+        Su[i] = m.gu[SYM[i][0]] * Sl[0] + m.gu[SYM[i][1]] * Sl[1] + m.gu[SYM[i][2]] * Sl[2];
+        Bl[i] = lower(m, B, i);
+    }
+    const double S2 = Sl[0] * Su[0] + Sl[1] * Su[1] + Sl[2] * Su[2];
+    const double B2 = Bl[0] * B[0] + Bl[1] * B[1] + Bl[2] * B[2];
+    const double SB = Sl[0] * B[0] + Sl[1] * B[1] + Sl[2] * B[2];
+    const double E = tau + D;
+    auto eval = [&](double z, double& W, double& rho, double& p) {
+        double v2 = (S2 * z * z + SB * SB * (B2 + 2.0 * z)) / ((z + B2) * (z + B2) * z * z);
+        if (v2 > 1.0 - 1e-15) v2 = 1.0 - 1e-15;
+        W = 1.0 / std::sqrt(1.0 - v2);
+        rho = D / W;
+        p = (gamma - 1.0) / gamma * (z / (W * W) - rho);
+        return z + B2 - p - B2 / (2.0 * W * W) - SB * SB / (2.0 * z * z) - E;
+    };
+    // bracket: f is increasing in z for physical states
+    double W, rho, p;
+    double zlo = 1e-300, zhi = std::fmax(2.0 * (E + 1.0), 1.0);
+    for (int it = 0; it < 200 && eval(zhi, W, rho, p) < 0.0; ++it) zhi *= 2.0;
+    zlo = zhi;
+    for (int it = 0; it < 400 && eval(zlo, W, rho, p) > 0.0; ++it) zlo *= 0.5;
+    double z = 0.5 * (zlo + zhi);
+    int status = 1;
+    for (int it = 0; it < 200; ++it) {
+        double f = eval(z, W, rho, p);
+        if (f > 0.0) zhi = z; else zlo = z;
+        const double h = 1e-6 * z;
+        double fp = (eval(z + h, W, rho, p) - eval(z - h, W, rho, p)) / (2.0 * h);
+        double zn = z - f / fp;
+        if (!(zn > zlo && zn < zhi)) zn = 0.5 * (zlo + zhi);
+        const double dz = std::fabs(zn - z);
+        z = zn;
+        if (dz < 1e-14 * z) { status = 0; break; }
+    }
+    eval(z, W, rho, p);
+    P[0] = rho;
+    for (int i = 0; i < 3; ++i) P[1 + i] = (Su[i] + SB * B[i] / z) / (z + B2);
+    P[4] = p / ((gamma - 1.0) * rho);
+    for (int i = 0; i < 3; ++i) P[5 + i] = B[i];
+    return status;
+}
+
+}  // namespace
+
+// =================================================== C ABI ===================================================
+// All pointers are HOST pointers.  Array layout is the library's (include/grx.h): SoA, x fastest,
+// ghosts included, [box][field][k][j][i].  Return 0 = ok, 1 = invalid argument.
+extern "C" {
+
+int oracle_valencia_rhs(const int n[3], int nbox, const double* prim, const double* metric, const double* K,
+                        const double dx[3], int nghost, int recon, double gamma, double* out,
+                        unsigned long long* nfallback) {
+    return rhs_all<double>(n, nbox, prim, metric, K, dx, nghost, recon, gamma, out, nfallback, nullptr);
+}
+
+// adjudicator: same algorithm evaluated in long double (x87 80-bit), results rounded to double
+int oracle_valencia_rhs_ld(const int n[3], int nbox, const double* prim, const double* metric, const double* K,
+                           const double dx[3], int nghost, int recon, double gamma, double* out,
+                           unsigned long long* nfallback) {
+    return rhs_all<long double>(n, nbox, prim, metric, K, dx, nghost, recon, gamma, out, nfallback, nullptr);
+}
+
+// counting instance: ops[4] = {add/sub, mul, div, sqrt} executed by one whole call (compares, selects,
+// sign flips, abs and loads/stores are free).  Each face is evaluated once.
+int oracle_valencia_rhs_count(const int n[3], int nbox, const double* prim, const double* metric, const double* K,
+                              const double dx[3], int nghost, int recon, double gamma, double* out,
+                              unsigned long long ops[4]) {
+    OpCount c;
+    int rc = rhs_all<Counted>(n, nbox, prim, metric, K, dx, nghost, recon, gamma, out, nullptr, &c);
+    if (rc == 0 && ops) { ops[0] = c.add; ops[1] = c.mul; ops[2] = c.div; ops[3] = c.sqrt; }
+    return rc;
+}
+
+// O10: prim2con on ALL cells including ghosts, cell-centre metric (Eqs. 6-9)
+int oracle_prim2con(const int n[3], int nbox, const double* prim, const double* metric, int nghost, double gamma,
+                    double* cons) {
+    if (!n || !prim || !metric || !cons || nbox < 1 || nghost < 0 || !(gamma > 1.0)) return 1;
+    const size_t NC = (size_t)(n[0] + 2 * nghost) * (n[1] + 2 * nghost) * (n[2] + 2 * nghost);
+    for (int b = 0; b < nbox; ++b) {
+        const double* pb = prim + (size_t)b * 8 * NC;
+        const double* mb = metric + (size_t)b * 10 * NC;
+        double* cb = cons + (size_t)b * 8 * NC;
+#pragma omp parallel for schedule(static)
+        for (long c0 = 0; c0 < (long)NC; ++c0) {
+            Metric<double> m;
+            m.alp = mb[c0];
+            for (int a = 0; a < 3; ++a) m.beta[a] = mb[(1 + a) * NC + c0];
+            for (int c = 0; c < 6; ++c) m.g[c] = mb[(4 + c) * NC + c0];
+            metric_complete(m);
+            double P[8];
+            for (int q = 0; q < 8; ++q) P[q] = pb[q * NC + c0];
+            State<double> s;
+            prim2con_point(P, m, gamma, s);
+            for (int q = 0; q < 8; ++q) cb[q * NC + c0] = s.U[q];
+        }
+    }
+    return 0;
+}
+
+// support (R22): con2prim on all cells; returns the number of cells whose solve did not converge
+int oracle_con2prim(const int n[3], int nbox, const double* cons, const double* metric, int nghost, double gamma,
+                    double* prim) {
+    if (!n || !prim || !metric || !cons || nbox < 1 || nghost < 0 || !(gamma > 1.0)) return -1;
+    const size_t NC = (size_t)(n[0] + 2 * nghost) * (n[1] + 2 * nghost) * (n[2] + 2 * nghost);
+    int nfail = 0;
+    for (int b = 0; b < nbox; ++b) {
+        const double* cb = cons + (size_t)b * 8 * NC;
+        const double* mb = metric + (size_t)b * 10 * NC;
+        double* pb = prim + (size_t)b * 8 * NC;
+#pragma omp parallel for schedule(static) reduction(+ : nfail)
+        for (long c0 = 0; c0 < (long)NC; ++c0) {
+            Metric<double> m;
+            m.alp = mb[c0];
+            for (int a = 0; a < 3; ++a) m.beta[a] = mb[(1 + a) * NC + c0];
+            for (int c = 0; c < 6; ++c) m.g[c] = mb[(4 + c) * NC + c0];
+            metric_complete(m);
+            double U[8], P[8];
+            for (int q = 0; q < 8; ++q) U[q] = cb[q * NC + c0];
+            nfail += con2prim_point(U, m, gamma, P);
+            for (int q = 0; q < 8; ++q) pb[q * NC + c0] = P[q];
+        }
+    }
+    return nfail;
+}
+
+// ---- point-level entry points used by the pins (tests/test_oracle_pins*.py) -------------------------
+void oracle_recon_cell(int recon, const double q[5], double* qm, double* qp) {
+    recon_cell<double>(recon, q[0], q[1], q[2], q[3], q[4], *qm, *qp);
+}
+
+static void fill_metric(Metric<double>& m, const double met[10]) {
+    m.alp = met[0];
+    for (int a = 0; a < 3; ++a) m.beta[a] = met[1 + a];
+    for (int c = 0; c < 6; ++c) m.g[c] = met[4 + c];
+}
+
+// U, F^d and the two characteristic speeds of one state in one metric (O4-O6)
+void oracle_state_flux(const double P[8], const double met[10], int d, double gamma, double U[8], double F[8],
+                       double lam[2]) {
+    Metric<double> m;
+    fill_metric(m, met);
+    metric_complete(m);
+    State<double> s;
+    prim2con_point(P, m, gamma, s);
+    for (int c = 0; c < 8; ++c) U[c] = s.U[c];
+    flux_point(P, m, s, d, F);
+    wavespeeds_point(P, m, s, d, gamma, lam[0], lam[1]);
+}
+
+// HLLE flux of one interface from already reconstructed states and an already averaged face metric (O3-O7)
+void oracle_face_flux(const double PL[8], const double PR[8], const double CL[8], const double CR[8],
+                      const double met_face[10], int d, double gamma, double Fh[8]) {
+    Metric<double> m;
+    fill_metric(m, met_face);
+    face_flux(m, d, gamma, PL, PR, CL, CR, Fh, nullptr);
+}
+
+void oracle_hlle(const double UL[8], const double FL[8], const double lamL[2], const double UR[8],
+                 const double FR[8], const double lamR[2], double Fh[8]) {
+    hlle<double>(UL, FL, lamL[0], lamL[1], UR, FR, lamR[0], lamR[1], Fh);
+}
+
+// sources of one cell from point values and given metric derivatives dm[3][10] (O9)
+void oracle_sources_point(const double P[8], const double met[10], const double K[6], const double dm[30],
+                          double gamma, double S[8]) {
+    Metric<double> m;
+    fill_metric(m, met);
+    double d3[3][10];
+    for (int a = 0; a < 3; ++a)
+        for (int f = 0; f < 10; ++f) d3[a][f] = dm[a * 10 + f];
+    sources_point(P, m, K, d3, gamma, S);
+}
+
+double oracle_weno_eps(void) { return WENO_EPS; }
+double oracle_v2max(void) { return V2MAX; }
+
+}  // extern "C"
