@@ -1,0 +1,430 @@
+#!/usr/bin/env python
+"""bench.py -- FP64 Valencia RHS cell-updates/s on one 256^3 block (WENO5 + HLLE), B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c5-256]
+                    [--recon weno5|minmod|mc] [--sweep]
+
+A "step" is ONE evaluation of the whole hot path (reconstruct -> HLLE -> flux divergence + sources, all three
+directions) over one batch of synthetic input, i.e. one grx_valencia_rhs call = one
+kernel launch.  Workload at N=1: config 5's 256^3 x 1 box (the configuration BASELINE.json's metric is quoted
+on: "WENO5+HLLE, 256^3"), seeded smooth random state on a perturbed conformally flat metric with shift and
+K_ij (inputs.sweep_boxes).  Inputs (4.6 GB) are far larger than the 126 MB L2, so no flush between steps.
+With N>1 (torchrun) every rank evaluates its own block of the same shape (weak scaling, no data-path
+collective: the path partitions over blocks); time = max over ranks.
+
+Prints ONE JSON line (rank 0).  `value` = interior cells x boxes x ranks x steps / time, inputs resident in
+HBM; `e2e` = same through grx_valencia_rhs_host with pinned HOST buffers (H2D of all inputs and D2H of the
+result inside the timed region); `roofline` = algorithmic FP64 flops of the launch (the oracle's counted
+operations) / kernel time against the FP64 peak, plus the HBM view; `cpu_baseline` =
+the oracle, as it stands, on the host cores on a bounded sub-block of the same workload.
+
+--impl reference times the oracle (the only reference there is: the paper ships no code) on this host.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2210_17509_b200 import inputs  # noqa: E402
+
+METRIC = "FP64 Valencia RHS cell-updates/sec (WENO5+HLLE, 256^3)"
+UNIT = "cell-updates/s"
+
+# Algorithmic flops per cell-update of a cubic N^3 box = A + B/N: the operation count of the oracle's
+# counting instance (add = mul = div = sqrt = 1, an FMA would be 2; every face once), fitted on
+# N = 16, 32, 48 general-metric boxes (oracle/count_flops.py; tests/test_bench_model.py re-checks it).
+FLOPS_MODEL = {"weno5": (4753.0, 6209.0), "minmod": (2545.0, 1793.0), "mc": (2640.0, 1500.0)}
+# Nominal FP64 peak of a B200: 148 SMs x 64 FP64 lanes x 2 flop (FMA) x 1.965 GHz.
+FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+
+
+def algorithmic_flops_per_cell(n, recon):
+    a, b = FLOPS_MODEL[recon]
+    return a + (b / 3.0) * (1.0 / n[0] + 1.0 / n[1] + 1.0 / n[2])
+
+
+def algorithmic_bytes_per_cell(n, g):
+    """24 input fields read once including ghosts + 8 output fields written on the interior."""
+    tot = (n[0] + 2 * g) * (n[1] + 2 * g) * (n[2] + 2 * g)
+    return 8.0 * (24.0 * tot / (n[0] * n[1] * n[2]) + 8.0)
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except OSError:
+        return {"hbm_gbs": 6650.0}, "fallback"
+
+
+# ------------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU with NVML while a region runs."""
+
+    def __init__(self, index, period=0.01):
+        self.index, self.period = index, period
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
+        self._h = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+        except Exception:   # NVML not usable: clocks are reported as unknown
+            self._h = None
+
+    _NAMES = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+              0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+              0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self._h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+                for bit, name in self._NAMES.items():
+                    if r & bit and name != "gpu_idle":
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def __enter__(self):
+        if self._h is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thread:
+            self._thread.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------ oracle legs
+def _sub_block(prob, nz_sub, ny_sub=None, nx_sub=None):
+    """First nx_sub x ny_sub x nz_sub interior cells of box 0 with their ghost shell (a bounded sample of the
+    same workload: the right-hand side of a cell only depends on cells within 3 of it)."""
+    g = prob.nghost
+    nx = min(nx_sub or prob.n[0], prob.n[0])
+    ny = min(ny_sub or prob.n[1], prob.n[1])
+    nz = min(nz_sub, prob.n[2])
+    sl = (slice(0, 1), slice(None), slice(0, nz + 2 * g), slice(0, ny + 2 * g), slice(0, nx + 2 * g))
+    return [np.ascontiguousarray(a[sl]) for a in (prob.prim, prob.metric, prob.K)], (nx, ny, nz)
+
+
+def time_oracle(prob, recon, budget_s, reps=1):
+    """Times the oracle (as it stands) on a sub-block sized for about `budget_s` seconds per repetition."""
+    from oracle import oracle as orc
+    orc.lib()
+    (p, m, k), n0 = _sub_block(prob, 8, 64, 64)
+    t0 = time.perf_counter()
+    orc.valencia_rhs(p, m, k, prob.dx, prob.nghost, recon, prob.gamma)
+    rate = n0[0] * n0[1] * n0[2] / max(time.perf_counter() - t0, 1e-6)    # calibration, cold
+    want = max(rate * budget_s, 4096.0)
+    nx, ny = prob.n[0], prob.n[1]
+    nz = int(min(prob.n[2], max(1, want // (nx * ny))))
+    if nz == 1 and want < nx * ny:
+        ny = int(max(1, want // nx))
+    (p, m, k), n1 = _sub_block(prob, nz, ny, nx)
+    cells = n1[0] * n1[1] * n1[2]
+    best = None
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        orc.valencia_rhs(p, m, k, prob.dx, prob.nghost, recon, prob.gamma)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return cells / best, best, n1, orc.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    prob = load_workload(args.workload, 0)
+    from oracle import oracle as orc
+    orc.lib()
+    total_budget = 100.0
+    per_step = total_budget / (args.steps + args.warmup)
+    # one calibration inside time_oracle, then the same sub-block every step
+    (p0, m0, k0), n0 = _sub_block(prob, 8, 64, 64)
+    t0 = time.perf_counter()
+    orc.valencia_rhs(p0, m0, k0, prob.dx, prob.nghost, args.recon, prob.gamma)
+    rate = n0[0] * n0[1] * n0[2] / max(time.perf_counter() - t0, 1e-6)
+    want = max(rate * per_step, 4096.0)
+    nz = int(min(prob.n[2], max(1, want // (prob.n[0] * prob.n[1]))))
+    ny = prob.n[1] if want >= prob.n[0] * prob.n[1] else int(max(1, want // prob.n[0]))
+    (p, m, k), n1 = _sub_block(prob, nz, ny, prob.n[0])
+    cells = n1[0] * n1[1] * n1[2]
+    for _ in range(args.warmup):
+        orc.valencia_rhs(p, m, k, prob.dx, prob.nghost, args.recon, prob.gamma)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.valencia_rhs(p, m, k, prob.dx, prob.nghost, args.recon, prob.gamma)
+    dt = time.perf_counter() - t0
+    value = cells * args.steps / dt
+    sample = f"first {n1[0]}x{n1[1]}x{n1[2]} interior cells (+3 ghosts) of the {prob.name} block, per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{prob.name}, {args.recon}+HLLE, Gamma-law, general metric + K_ij; oracle on host cores",
+                   "l2": "n/a (CPU)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ GPU arm
+def load_workload(name, rank):
+    if name.startswith("c5-"):
+        N = int(name[3:])
+        nbox = dict(inputs.SWEEP).get(N, 1)
+        if rank == 0:
+            return inputs.sweep_boxes(N, nbox)
+        # other ranks: same shapes, their own seeds (boxes rank*nbox .. rank*nbox+nbox-1 of the same family)
+        prims, mets, Ks = [], [], []
+        for b in range(nbox):
+            prim, met, K, dx, gamma = inputs._smooth_box(N, 1000 * N + rank * nbox + b, inputs.NGHOST)
+            prims.append(prim), mets.append(met), Ks.append(K)
+        return inputs.Problem(f"C5-{N}^3x{nbox}", (N, N, N), nbox, inputs.NGHOST, dx, gamma, np.stack(prims),
+                              np.stack(mets), np.stack(Ks), ("minmod", "weno5"))
+    return inputs.by_name(name)
+
+
+def time_rhs(grx, torch, prob, dev, recon, steps, warmup, stream):
+    prim, met, K = dev
+    out = torch.empty_like(prim)
+    for _ in range(warmup):
+        grx.valencia_rhs(prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, out=out, stream=stream)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stream.synchronize()
+    e0.record(stream)
+    for _ in range(steps):
+        grx.valencia_rhs(prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, out=out, stream=stream)
+    e1.record(stream)
+    stream.synchronize()
+    return e0.elapsed_time(e1) * 1e-3, out
+
+
+def measure_dfma_peak(grx, torch, stream):
+    sink = torch.zeros(1, dtype=torch.float64, device="cuda")
+    grx.dfma_peak_launch(2000, sink, stream)
+    best = 0.0
+    for _ in range(5):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        flops = grx.dfma_peak_launch(20000, sink, stream)
+        e1.record(stream)
+        stream.synchronize()
+        best = max(best, flops / (e0.elapsed_time(e1) * 1e-3))
+    return best / 1e12
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2210_17509_b200 import build, grx
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    grx.lib()
+    stream = torch.cuda.current_stream()
+
+    prob = load_workload(args.workload, rank)
+    recon = args.recon
+    host = [torch.from_numpy(np.ascontiguousarray(a)) for a in (prob.prim, prob.metric, prob.K)]
+    dev = tuple(t.cuda() for t in host)
+    cells = prob.cells
+    g = prob.nghost
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident timing (the headline `value`), clocks sampled during it
+    time_rhs(grx, torch, prob, dev, recon, 0, max(args.warmup, 3), stream)
+    barrier()
+    with ClockSampler(local) as cs:
+        t_dev, out = time_rhs(grx, torch, prob, dev, recon, args.steps, 0, stream)
+        barrier()
+    clocks = cs.summary()
+    if clocks["samples"] < 5:
+        # timed region too short for NVML's sampling period: sample the same kernel over >= 0.5 s (untimed)
+        n_extra = int(max(10, 0.6 / max(t_dev / args.steps, 1e-6)))
+        with ClockSampler(local) as cs2:
+            time_rhs(grx, torch, prob, dev, recon, n_extra, 0, stream)
+        c2 = cs2.summary()
+        c2["note"] = "sampled over an untimed repeat of the timed kernel (timed region shorter than the NVML period)"
+        clocks = c2
+    tt = torch.tensor([t_dev], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_max = float(tt.item())
+    value = cells * world * args.steps / t_max
+
+    # ---- end to end through grx_valencia_rhs_host: pinned host buffers, H2D + kernel + D2H per step
+    e2e_steps = max(1, min(args.steps, 5))
+    hp, hm, hk = (t.pin_memory() for t in host)
+    ho = torch.empty_like(hp).pin_memory()
+    ws = torch.empty(grx.host_workspace_bytes(hp.shape, g) // 8, dtype=torch.float64, device="cuda")
+    grx.valencia_rhs_host(hp, hm, hk, prob.dx, g, recon, prob.gamma, ho, ws, stream=stream)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        grx.valencia_rhs_host(hp, hm, hk, prob.dx, g, recon, prob.gamma, ho, ws, stream=stream)
+    e1.record(stream)
+    stream.synchronize()
+    te = torch.tensor([e0.elapsed_time(e1) * 1e-3], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = cells * world * e2e_steps / float(te.item())
+    e2e_ok = bool(np.array_equal(ho.numpy()[prob.interior], out.cpu().numpy()[prob.interior]))
+    h2d = int(sum(t.numel() for t in (hp, hm, hk)) * 8)
+    d2h = int(ho.numel() * 8)
+    del ws, hp, hm, hk, ho
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the (single) kernel of a step; its launch duration = step time (one launch per step)
+    peaks, peak_src = measured_peaks()
+    t_launch = t_dev / args.steps
+    fl_cell = algorithmic_flops_per_cell(prob.n, recon)
+    by_cell = algorithmic_bytes_per_cell(prob.n, g)
+    ach_tflops = fl_cell * cells / t_launch / 1e12
+    ach_gbs = by_cell * cells / t_launch / 1e9
+    dfma = measure_dfma_peak(grx, torch, stream)
+    roofline = {
+        "bound": "alu", "kernel": "rhs_fused_kernel", "achieved": ach_tflops, "peak": FP64_PEAK_NOMINAL_TFLOPS,
+        "unit": "TFLOP/s", "frac": ach_tflops / FP64_PEAK_NOMINAL_TFLOPS,
+        "peak_source": "nominal FP64: 148 SM x 64 lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry)",
+        "peak_dfma_measured": dfma, "frac_of_dfma_measured": ach_tflops / dfma if dfma > 0 else None,
+        "flops_per_cell": fl_cell, "bytes_per_cell": by_cell,
+        "hbm": {"achieved": ach_gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s", "peak_source": peak_src,
+                "frac": ach_gbs / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None},
+        "traffic": None,
+    }
+    tr = os.path.join(ROOT, "profiles", "traffic_bytes_per_launch.json")
+    if os.path.exists(tr):
+        try:
+            with open(tr) as f:
+                roofline["traffic"] = json.load(f).get(f"{args.workload}/{recon}")
+        except (OSError, ValueError):
+            pass
+
+    # ---- the oracle on the host cores, bounded sample of the same workload
+    cpu_rate, cpu_t, n1, cores = time_oracle(prob, recon, budget_s=args.cpu_seconds)
+    cpu_baseline = {"value": cpu_rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                    "sample": f"first {n1[0]}x{n1[1]}x{n1[2]} interior cells (+3 ghosts) of the same block, "
+                              f"one evaluation, {cpu_t:.1f} s"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{prob.name} per GPU, {recon}+HLLE, Gamma-law EOS, perturbed conformally flat metric "
+                               f"+ shift + K_ij, {g} ghosts; one grx_valencia_rhs call per step",
+                   "l2": "inputs 4.6 GB >> 126 MB L2, no flush", "tile": os.environ.get("GRX_TILE", "default"),
+                   "parallelism": f"blocks x{world}, no collective"},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": e2e_steps, "matches_device_path": e2e_ok},
+        "gpu_launches": args.steps,
+        "roofline": roofline,
+        "cpu_baseline": cpu_baseline,
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def run_sweep(args):
+    """Config-5 sweep + the other configs: one JSON line per point (not the driver's contract line)."""
+    import torch
+    from paper_2210_17509_b200 import build, grx
+    build.build()
+    grx.lib()
+    stream = torch.cuda.current_stream()
+    for name in ("c5-32", "c5-64", "c5-128", "c5-256", "c4", "c3", "c2", "c1"):
+        prob = load_workload(name, 0)
+        dev = tuple(torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (prob.prim, prob.metric, prob.K))
+        for recon in prob.recons:
+            t, _ = time_rhs(grx, torch, prob, dev, recon, args.steps, max(args.warmup, 3), stream)
+            tl = t / args.steps
+            fl = algorithmic_flops_per_cell(prob.n, recon) * prob.cells / tl / 1e12
+            gb = algorithmic_bytes_per_cell(prob.n, prob.nghost) * prob.cells / tl / 1e9
+            print(json.dumps({"workload": prob.name, "recon": recon, "cells": prob.cells, "us_per_call": 1e6 * tl,
+                              "cell_updates_per_s": prob.cells / tl, "tflops_alg": fl,
+                              "frac_fp64_nominal": fl / FP64_PEAK_NOMINAL_TFLOPS, "gbs_alg": gb,
+                              "tile": os.environ.get("GRX_TILE", "default")}), flush=True)
+        del dev
+        torch.cuda.empty_cache()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c5-256")
+    ap.add_argument("--recon", default="weno5", choices=["weno5", "minmod", "mc"])
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="wall-clock budget of the oracle sample")
+    ap.add_argument("--sweep", action="store_true", help="time every config instead of the contract line")
+    args = ap.parse_args()
+    if args.steps < 1:
+        raise SystemExit("--steps must be >= 1")
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

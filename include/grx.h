@@ -1,0 +1,141 @@
+/* grx.h -- C ABI of the B200-native FP64 Valencia GRMHD right-hand side.
+ *
+ * The method is the right-hand-side evaluation of GRaM-X (arxiv 2210.17509; citations are PAPER.md
+ * line numbers): "reconstruct -> Riemann -> flux divergence + source" (steps 2-4, l.127-132) of the
+ * Valencia formulation, Eqs. (6)-(13) (l.86-114), with TVD/WENO5 reconstruction (l.130, l.134), the
+ * HLLE solver (l.131, l.136) and an ideal-gas Gamma-law EOS (l.138).  Readings of everything the paper
+ * leaves open (R1..R29) are listed in DESIGN.md.
+ *
+ * Conventions shared by every entry point
+ * ---------------------------------------
+ *  - Every array pointer is a DEVICE pointer to FP64 unless it says HOST.  The caller owns all memory;
+ *    the library never allocates, frees or keeps user memory, holds no state between calls, and needs
+ *    no workspace.
+ *  - Layout: structure of arrays, x fastest, ghost zones included, boxes contiguous:
+ *        a[box][field][k][j][i],   i in [0,Nx), j in [0,Ny), k in [0,Nz),   N* = n* + 2*nghost,
+ *    interior cell (i,j,k) of the paper's block (l.184) sits at (i+nghost, j+nghost, k+nghost).
+ *  - Fields (fixed order):
+ *        prim  [8] : rho, v^x, v^y, v^z, eps, B^x, B^y, B^z     (P of l.118; Valencia v^i, Eq. 10 l.98;
+ *                                                               eps = specific internal energy, R1)
+ *        metric[10]: alp, beta^x, beta^y, beta^z, g_xx, g_xy, g_xz, g_yy, g_yz, g_zz   (ADM, l.56)
+ *        K     [6] : K_xx, K_xy, K_xz, K_yy, K_yz, K_zz   (d_t g_ij = -2 alp K_ij + Lie_beta g_ij, R12)
+ *        cons/out[8]: D, S_x, S_y, S_z, tau, calB^x, calB^y, calB^z  (densitised, Eqs. 6-9 l.88-94)
+ *    Metric and K are co-located with the fluid at cell centres (R6).
+ *  - Calls are asynchronous on `cuda_stream` (a cudaStream_t; NULL = the legacy default stream); results
+ *    are valid after that stream is synchronised.
+ *  - Errors: every entry point returns a code, never aborts or throws.  Arguments are validated on the
+ *    host BEFORE any launch (nothing is written on GRX_ERR_INVALID_ARG).  CUDA launch failures map to
+ *    GRX_ERR_CUDA.  Inputs are not checked for physical admissibility on the device: an unphysical
+ *    cell-centre state gives NaN/Inf there, exactly as the equations do.
+ *  - There is NO CPU fallback: without a CUDA device every compute entry point returns GRX_ERR_CUDA.
+ */
+#ifndef GRX_H
+#define GRX_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+    int nx, ny, nz; /* interior cells per box, each >= 1                    */
+    int nbox;       /* boxes in this call, >= 1, stored back to back         */
+} grx_grid;
+
+enum { GRX_RECON_MINMOD = 0, GRX_RECON_MC = 1, GRX_RECON_WENO5 = 2 };
+enum { GRX_OK = 0, GRX_ERR_INVALID_ARG = 1, GRX_ERR_CUDA = 2, GRX_ERR_UNSUPPORTED = 3 };
+
+/* Kernel variants (grx_set_variant).  GRX_VARIANT_FUSED is the product path; GRX_VARIANT_SIMPLE is a
+ * one-thread-per-cell kernel that recomputes shared faces, kept as a cross-check of the fused one. */
+enum { GRX_VARIANT_FUSED = 0, GRX_VARIANT_SIMPLE = 1 };
+
+/* d/dt of the conserved variables on the interior cells of every box.
+ *
+ * Computes, per direction d = x,y,z:
+ *   face metric = 1/2 (cell- + cell+) (l.130, R6/R7); reconstruction of the 8 primitives to both sides of
+ *   every face with `recon` (minmod/MC: l.134, l.255; WENO5 Jiang-Shu: l.134, ref [32]); first-order
+ *   fallback of an inadmissible side (R5); conserved state Eqs. (6)-(10) and flux Eq. (12) per side
+ *   (l.88-108); fast-magnetosonic speeds (R8); HLLE flux (l.131, R9); out -= (F_{f+1} - F_f)/dx_d;
+ * then adds the geometric sources of Eq. (13) (l.112) in 3+1 form (R12-R14) with 4th-order centred
+ * metric derivatives, evaluated from the cell-centre primitives.
+ *
+ *   grid    HOST pointer.
+ *   prim    [nbox][8 ][Nz][Ny][Nx]  in.   Ghosts must be filled by the caller (l.170, l.222).
+ *   metric  [nbox][10][Nz][Ny][Nx]  in.
+ *   K       [nbox][6 ][Nz][Ny][Nx]  in.
+ *   dx      HOST pointer to 3 cell sizes, each > 0 (R11).
+ *   nghost  ghost width on every side: >= 3 for WENO5, >= 2 for minmod/MC (R29).
+ *   recon   GRX_RECON_*.
+ *   gamma   Gamma-law index, > 1 (l.138).
+ *   out     [nbox][8][Nz][Ny][Nx]   out.  Interior cells are overwritten; ghost cells are not touched
+ *           (R23).  Must not alias an input.
+ * Returns GRX_OK, GRX_ERR_INVALID_ARG (null pointer, n < 1, nbox < 1, nghost too small, unknown recon,
+ * gamma <= 1, dx <= 0, a box larger than 2^31-1 cells) or GRX_ERR_CUDA. */
+int grx_valencia_rhs(const grx_grid* grid, const double* prim, const double* metric, const double* K,
+                     const double dx[3], int nghost, int recon, double gamma, double* out, void* cuda_stream);
+
+/* Same computation for HOST arrays (end-to-end entry point): copies prim, metric and K to the device
+ * workspace, runs grx_valencia_rhs there and copies `out` back, all asynchronously on `cuda_stream`
+ * (cudaMemcpyAsync; the host arrays should be page-locked for the copies to be asynchronous).  The host
+ * arrays have the layout above.  The WHOLE out array is copied back (its ghost cells hold whatever the
+ * workspace held).
+ *   workspace        DEVICE pointer, at least grx_host_workspace_bytes(grid, nghost) bytes, owned by the caller.
+ * Results are valid in out_host after the stream is synchronised. */
+size_t grx_host_workspace_bytes(const grx_grid* grid, int nghost);
+int grx_valencia_rhs_host(const grx_grid* grid, const double* prim_host, const double* metric_host,
+                          const double* K_host, const double dx[3], int nghost, int recon, double gamma,
+                          double* out_host, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Conserved variables from the primitives, Eqs. (6)-(9), with the CELL-CENTRE metric,
+ * on ALL cells including ghosts (step 2 of the initialisation, l.120-123).
+ *   cons    [nbox][8][Nz][Ny][Nx]   out.  nghost >= 0. */
+int grx_prim2con(const grx_grid* grid, const double* prim, const double* metric, int nghost, double gamma,
+                 double* cons, void* cuda_stream);
+
+/* SUPPORT CODE for short evolutions (R21/R22; not on the graded path): primitives from conserved
+ * variables for the Gamma-law EOS by a bracketed Newton solve in z = rho h W^2 (stand-in for the paper's
+ * 3D-NR scheme, l.142-146), on ALL cells including ghosts.
+ *   prim    [nbox][8][Nz][Ny][Nx]   out.
+ *   nfail   DEVICE pointer to one unsigned long long, or NULL: incremented (atomically) by the number of
+ *           cells whose solve did not converge; the caller zeroes it. */
+int grx_con2prim(const grx_grid* grid, const double* cons, const double* metric, int nghost, double gamma,
+                 double* prim, unsigned long long* nfail, void* cuda_stream);
+
+/* SUPPORT CODE: y[interior] = a*x[interior] + b*(y[interior] + dt*rhs[interior]) on 8-field arrays --
+ * the building block of the SSP-RK2 stages (l.125, R21).  x may equal y. */
+int grx_rk_axpy(const grx_grid* grid, int nghost, double a, const double* x, double b, double dt,
+                const double* rhs, double* y, void* cuda_stream);
+
+/* Debug: if `counter` (DEVICE pointer to one unsigned long long, caller-zeroed) is non-NULL, later
+ * grx_valencia_rhs calls of this host thread add to it the number of face sides that took the R5
+ * first-order fallback.  NULL switches counting off (the default; counting costs a few atomics). */
+int grx_debug_set_fallback_counter(unsigned long long* counter);
+
+/* Selects the kernel variant used by later grx_valencia_rhs calls of this process (default FUSED). */
+int grx_set_variant(int variant);
+
+/* Accuracy self-test of the division-free reciprocal / rsqrt / sqrt helpers the kernels use:
+ * y[0..n) = 1/x, y[n..2n) = 1/sqrt(x), y[2n..3n) = sqrt(x) for x[0..n) > 0 (DEVICE pointers). */
+int grx_selftest_math(const double* x, double* y, size_t n, void* cuda_stream);
+
+/* Throughput of a dependent-chain-free DFMA loop on the whole device: launches the micro-benchmark
+ * kernel once (iters FMAs per chain, 8 chains per thread, one resident wave) and writes a checksum to
+ * `sink` (DEVICE pointer to one double).  flops_out (HOST) receives the flop count of that launch; time
+ * it with CUDA events on `cuda_stream` to obtain the FP64 peak used as the roofline denominator. */
+int grx_dfma_peak_launch(int iters, double* sink, double* flops_out, void* cuda_stream);
+
+/* Thread-local description of the last non-OK return of this thread ("" if none). */
+const char* grx_last_error(void);
+
+/* Library version: major*10000 + minor*100 + patch. */
+int grx_version(void);
+
+/* Compile-time conventions (R4, R5), exported so tests can assert that both implementations agree. */
+double grx_weno_eps(void);
+double grx_v2max(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRX_H */

@@ -1,0 +1,176 @@
+// grx_api.cu -- the C ABI of include/grx.h: argument validation on the host, launch geometry, error mapping.
+// No torch types, no allocation, no state besides the kernel-variant switch and the debug counter pointer.
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+
+#include "../../include/grx.h"
+#include "grx_launch.h"
+
+namespace {
+
+thread_local char t_err[256] = "";
+thread_local unsigned long long* t_fallback_counter = nullptr;
+std::atomic<int> g_variant{GRX_VARIANT_FUSED};
+
+int fail(int code, const char* msg) {
+    std::snprintf(t_err, sizeof(t_err), "%s", msg);
+    return code;
+}
+int fail_cuda(cudaError_t e, const char* where) {
+    std::snprintf(t_err, sizeof(t_err), "%s: %s", where, cudaGetErrorString(e));
+    return GRX_ERR_CUDA;
+}
+
+// Fills the geometry part of RhsParams; returns nullptr if fine, else what is wrong.
+const char* make_geom(const grx_grid* grid, int nghost, grx::RhsParams& p) {
+    if (!grid) return "grid is NULL";
+    if (grid->nx < 1 || grid->ny < 1 || grid->nz < 1) return "grid: nx, ny, nz must be >= 1";
+    if (grid->nbox < 1 || grid->nbox > 65535) return "grid: nbox must be in [1, 65535]";
+    if (nghost < 0 || nghost > 1024) return "nghost out of range";
+    p.n[0] = grid->nx; p.n[1] = grid->ny; p.n[2] = grid->nz;
+    long long nc = 1;
+    for (int a = 0; a < 3; ++a) {
+        p.N[a] = p.n[a] + 2 * nghost;
+        nc *= p.N[a];
+        if (nc > 2147483647LL) return "a box (with ghosts) must not exceed 2^31-1 cells";
+    }
+    p.g = nghost;
+    p.nbox = grid->nbox;
+    p.nc = nc;
+    p.stride[0] = 1;
+    p.stride[1] = p.N[0];
+    p.stride[2] = (long long)p.N[0] * p.N[1];
+    return nullptr;
+}
+
+}  // namespace
+
+extern "C" {
+
+int grx_valencia_rhs(const grx_grid* grid, const double* prim, const double* metric, const double* K,
+                     const double dx[3], int nghost, int recon, double gamma, double* out, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim || !metric || !K || !dx || !out) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (recon != GRX_RECON_MINMOD && recon != GRX_RECON_MC && recon != GRX_RECON_WENO5)
+        return fail(GRX_ERR_INVALID_ARG, "unknown recon");
+    if (nghost < (recon == GRX_RECON_WENO5 ? 3 : 2))
+        return fail(GRX_ERR_INVALID_ARG, "nghost too small: WENO5 needs 3, minmod/MC need 2 (R29)");
+    if (!(gamma > 1.0)) return fail(GRX_ERR_INVALID_ARG, "gamma must be > 1");
+    for (int a = 0; a < 3; ++a) {
+        if (!(dx[a] > 0.0) || !(1.0 / dx[a] > 0.0)) return fail(GRX_ERR_INVALID_ARG, "dx must be > 0 and finite");
+        p.idx[a] = 1.0 / dx[a];
+    }
+    if (out == prim || out == metric || out == K) return fail(GRX_ERR_INVALID_ARG, "out must not alias an input");
+    p.prim = prim; p.met = metric; p.K = K; p.out = out;
+    p.gamma = gamma;
+    p.nfallback = t_fallback_counter;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const cudaError_t e = (g_variant.load() == GRX_VARIANT_SIMPLE) ? grx::launch_rhs_simple(p, recon, st)
+                                                                   : grx::launch_rhs_fused(p, recon, st);
+    if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs launch");
+    return GRX_OK;
+}
+
+size_t grx_host_workspace_bytes(const grx_grid* grid, int nghost) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (make_geom(grid, nghost, p)) return 0;
+    return (size_t)32 * (size_t)p.nc * (size_t)p.nbox * sizeof(double);
+}
+
+int grx_valencia_rhs_host(const grx_grid* grid, const double* prim_host, const double* metric_host,
+                          const double* K_host, const double dx[3], int nghost, int recon, double gamma,
+                          double* out_host, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim_host || !metric_host || !K_host || !out_host || !workspace)
+        return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    const size_t cells = (size_t)p.nc * (size_t)p.nbox;
+    if (workspace_bytes < 32 * cells * sizeof(double)) return fail(GRX_ERR_INVALID_ARG, "workspace too small");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    double* d_prim = static_cast<double*>(workspace);
+    double* d_met = d_prim + 8 * cells;
+    double* d_K = d_met + 10 * cells;
+    double* d_out = d_K + 6 * cells;
+    cudaError_t e = cudaMemcpyAsync(d_prim, prim_host, 8 * cells * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_met, metric_host, 10 * cells * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_K, K_host, 6 * cells * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_host H2D");
+    const int rc = grx_valencia_rhs(grid, d_prim, d_met, d_K, dx, nghost, recon, gamma, d_out, cuda_stream);
+    if (rc != GRX_OK) return rc;
+    e = cudaMemcpyAsync(out_host, d_out, 8 * cells * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_host D2H");
+    return GRX_OK;
+}
+
+int grx_prim2con(const grx_grid* grid, const double* prim, const double* metric, int nghost, double gamma,
+                 double* cons, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim || !metric || !cons) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (!(gamma > 1.0)) return fail(GRX_ERR_INVALID_ARG, "gamma must be > 1");
+    const cudaError_t e = grx::launch_prim2con(prim, metric, p.nc, p.nbox, gamma, cons, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_prim2con launch");
+    return GRX_OK;
+}
+
+int grx_con2prim(const grx_grid* grid, const double* cons, const double* metric, int nghost, double gamma,
+                 double* prim, unsigned long long* nfail, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim || !metric || !cons) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (!(gamma > 1.0)) return fail(GRX_ERR_INVALID_ARG, "gamma must be > 1");
+    const cudaError_t e =
+        grx::launch_con2prim(cons, metric, p.nc, p.nbox, gamma, prim, nfail, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_con2prim launch");
+    return GRX_OK;
+}
+
+int grx_rk_axpy(const grx_grid* grid, int nghost, double a, const double* x, double b, double dt, const double* rhs,
+                double* y, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!x || !rhs || !y) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    const cudaError_t e = grx::launch_rk_axpy(p, a, x, b, dt, rhs, y, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_rk_axpy launch");
+    return GRX_OK;
+}
+
+int grx_debug_set_fallback_counter(unsigned long long* counter) {
+    t_fallback_counter = counter;
+    return GRX_OK;
+}
+
+int grx_set_variant(int variant) {
+    if (variant != GRX_VARIANT_FUSED && variant != GRX_VARIANT_SIMPLE) return fail(GRX_ERR_INVALID_ARG, "unknown variant");
+    g_variant.store(variant);
+    return GRX_OK;
+}
+
+int grx_selftest_math(const double* x, double* y, size_t n, void* cuda_stream) {
+    if (n && (!x || !y)) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    const cudaError_t e = grx::launch_selftest_math(x, y, n, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_selftest_math launch");
+    return GRX_OK;
+}
+
+int grx_dfma_peak_launch(int iters, double* sink, double* flops_out, void* cuda_stream) {
+    if (iters < 1 || !sink) return fail(GRX_ERR_INVALID_ARG, "iters must be >= 1 and sink non-NULL");
+    const cudaError_t e = grx::launch_dfma_peak(iters, sink, flops_out, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_dfma_peak_launch");
+    return GRX_OK;
+}
+
+const char* grx_last_error(void) { return t_err; }
+int grx_version(void) { return 100; }   /* 0.1.0 */
+double grx_weno_eps(void) { return grx::WENO_EPS; }
+double grx_v2max(void) { return grx::V2MAX; }
+
+}  // extern "C"

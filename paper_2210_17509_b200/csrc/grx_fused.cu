@@ -1,0 +1,307 @@
+// grx_fused.cu -- the product kernel: reconstruct + HLLE + flux divergence in all three directions and the
+// geometric sources in ONE pass over the block (steps 2-4), every face flux computed
+// exactly once.
+//
+// Decomposition:
+//   * A CTA owns an in-plane tile of TX x TY cells (TX = 32 = one warp along x, TY warps along y) and
+//     MARCHES along z through a chunk of the block, one plane per step.
+//   * z-direction: each thread reconstructs its own cell along z and keeps q^+ of the previous plane in
+//     registers, so the face k-1/2 is evaluated once, by the thread that owns the column; the finished
+//     right-hand side of cell k-1 is stored at step k.
+//   * x- and y-direction: every thread reconstructs its own cell, publishes q^+ in shared memory, evaluates
+//     the face on its low side (from its neighbour's q^+ and its own q^-), publishes the flux, and takes the
+//     flux of its high face from its neighbour.  The faces and one-sided reconstructions on the rim of the
+//     tile belong to one extra "rim warp" per CTA, whose lanes run along the tile edges.
+//   * Sources: metric derivatives and the 3+1 source terms per cell, added to the same accumulators.
+// Global loads go through L1/L2 (__ldg); lanes run along x, so every load is a contiguous 256 B row segment.
+#include <cstdio>
+#include <cstdlib>
+
+#include "grx_launch.h"
+
+namespace grx {
+
+constexpr int TX = 32;
+
+struct TileGeom {
+    int ntx, nty, nzc, tz;   // tiles along x, y; z-chunks and their length
+};
+
+// shared-memory exchange buffer: [8 fields][TY+1 rows][TX+1 columns]
+template <int TY>
+struct Exch {
+    double v[8][TY + 1][TX + 1];
+};
+
+// Reconstruct the 8 primitives of cell c along a direction with element stride s.
+template <int RECON>
+__device__ __forceinline__ void recon8(const double* __restrict__ prim, long long nc, long long c, long long s,
+                                       double qm[8], double qp[8]) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const double* f = prim + q * nc + c;
+        double a = 0.0, e = 0.0;
+        if (RECON == RECON_WENO5) { a = ldg(f - 2 * s); e = ldg(f + 2 * s); }
+        recon_cell<RECON>(a, ldg(f - s), ldg(f), ldg(f + s), e, qm[q], qp[q]);
+    }
+}
+
+// HLLE flux of the face between cells iL and iR = iL + s from given left/right states.
+template <int D>
+__device__ __forceinline__ void face8(const double* __restrict__ prim, const double* __restrict__ met, long long nc,
+                                      long long iL, long long iR, const double PL[8], const double PR[8], double gamma,
+                                      double Fh[8], unsigned& nfb) {
+    FaceGeom m;
+    m.alp = 0.5 * (ldg(met + iL) + ldg(met + iR));
+#pragma unroll
+    for (int a = 0; a < 3; ++a) m.beta[a] = 0.5 * (ldg(met + (1 + a) * nc + iL) + ldg(met + (1 + a) * nc + iR));
+#pragma unroll
+    for (int c = 0; c < 6; ++c) m.g[c] = 0.5 * (ldg(met + (4 + c) * nc + iL) + ldg(met + (4 + c) * nc + iR));
+    face_flux<D>(m, PL, PR, prim + iL, prim + iR, nc, gamma, Fh, nfb);
+}
+
+template <int RECON, int TY, int MINB>
+__global__ void __launch_bounds__((TY + 1) * 32, MINB)
+rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
+    extern __shared__ double smem_raw[];
+    Exch<TY>& Qb = *reinterpret_cast<Exch<TY>*>(smem_raw);
+    Exch<TY>& Fb = *reinterpret_cast<Exch<TY>*>(smem_raw + sizeof(Exch<TY>) / sizeof(double));
+
+    int t = blockIdx.x;
+    const int tix = t % tg.ntx; t /= tg.ntx;
+    const int tiy = t % tg.nty; t /= tg.nty;
+    const int zc = t;
+    const int box = blockIdx.y;
+    const int X0 = tix * TX, Y0 = tiy * TY, k0 = zc * tg.tz;
+    const int txe = min(TX, p.n[0] - X0), tye = min(TY, p.n[1] - Y0);
+    const int nk = min(tg.tz, p.n[2] - k0);       // planes owned by this CTA
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    const double* __restrict__ prim = p.prim + (long long)box * 8 * p.nc;
+    const double* __restrict__ met = p.met + (long long)box * 10 * p.nc;
+    const double* __restrict__ Kf = p.K + (long long)box * 6 * p.nc;
+    double* __restrict__ out = p.out + (long long)box * 8 * p.nc;
+    const long long nc = p.nc, sy = p.stride[1], sz = p.stride[2];
+    const double gamma = p.gamma;
+    const long long cbase = (X0 + p.g) + sy * (Y0 + p.g) + sz * (k0 - 1 + p.g);   // tile origin, plane k0-1
+    unsigned nfb = 0;
+
+    if (warp < TY) {
+        // ------------------------------------------------ regular warp: one cell column per thread
+        const bool active = (lane < txe) && (warp < tye);
+        long long c = cbase + lane + sy * warp;
+        double qpz[8], acc[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { qpz[q] = 0.0; acc[q] = 0.0; }
+        for (int kk = -1; kk <= nk; ++kk, c += sz) {
+            if (active) {
+                // z: reconstruct this cell, close the face below it, finish the cell below
+                double qm[8], qp[8];
+                recon8<RECON>(prim, nc, c, sz, qm, qp);
+                if (kk >= 0) {
+                    double Fh[8];
+                    // the first face of an inner chunk is also the last face of the chunk below: count once
+                    unsigned dup = 0;
+                    face8<2>(prim, met, nc, c - sz, c, qpz, qm, gamma, Fh, (kk == 0 && k0 > 0) ? dup : nfb);
+                    // F/dz is rounded once and used with both signs, so a uniform state cancels exactly
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) Fh[q] = __dmul_rn(Fh[q], p.idx[2]);
+                    if (kk >= 1) {
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) out[q * nc + c - sz] = __dsub_rn(acc[q], Fh[q]);
+                    }
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) acc[q] = Fh[q];
+                }
+#pragma unroll
+                for (int q = 0; q < 8; ++q) qpz[q] = qp[q];
+            }
+            if (kk < 0 || kk >= nk) continue;   // uniform over the CTA
+            // x
+            double qm[8];
+            if (active) {
+                double qp[8];
+                recon8<RECON>(prim, nc, c, 1, qm, qp);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) Qb.v[q][warp][lane + 1] = qp[q];
+            }
+            __syncthreads();
+            if (active) {
+                double PL[8], Fh[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][warp][lane];
+                face8<0>(prim, met, nc, c - 1, c, PL, qm, gamma, Fh, nfb);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) Fb.v[q][warp][lane] = Fh[q];
+            }
+            __syncthreads();
+            // y
+            if (active) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) acc[q] = fma(Fb.v[q][warp][lane] - Fb.v[q][warp][lane + 1], p.idx[0], acc[q]);
+                double qp[8];
+                recon8<RECON>(prim, nc, c, sy, qm, qp);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) Qb.v[q][warp + 1][lane] = qp[q];
+            }
+            __syncthreads();
+            if (active) {
+                double PL[8], Fh[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][warp][lane];
+                face8<1>(prim, met, nc, c - sy, c, PL, qm, gamma, Fh, nfb);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) Fb.v[q][warp][lane] = Fh[q];
+            }
+            __syncthreads();
+            if (active) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) acc[q] = fma(Fb.v[q][warp][lane] - Fb.v[q][warp + 1][lane], p.idx[1], acc[q]);
+                double s1, s2, s3, s4;
+                sources_from_global(p, prim, met, Kf, c, s1, s2, s3, s4);
+                acc[1] += s1; acc[2] += s2; acc[3] += s3; acc[4] += s4;
+            }
+        }
+    } else {
+        // ------------------------------------------------ rim warp: the tile's edge work
+        // x-rim: lane l < tye          -> cell (X0-1,   Y0+l): its q^+ feeds the first face of row l
+        //        lane TY + l, l < tye  -> cell (X0+txe, Y0+l): its q^- and the last face of row l
+        // y-rim: lane l < txe          -> cell (X0+l, Y0-1) [q^+] and cell (X0+l, Y0+tye) [q^-, last face of column l]
+        const bool xl = lane < tye;
+        const bool xr = (TY <= 16) && lane >= TY && (lane - TY) < tye;
+        const int xrow = xl ? lane : lane - TY;
+        const bool ycol = lane < txe;
+        for (int kk = 0; kk < nk; ++kk) {
+            const long long cp = cbase + sz * (kk + 1);   // tile origin in plane k0+kk
+            double yb_qp[8], yt_qm[8], xr_qm[8];
+            long long cxr = 0, cyt = 0;
+            if (ycol) {
+                double tmp[8];
+                recon8<RECON>(prim, nc, cp + lane - sy, sy, tmp, yb_qp);
+                cyt = cp + lane + sy * tye;
+                recon8<RECON>(prim, nc, cyt, sy, yt_qm, tmp);
+            }
+            if (xl || xr) {
+                double qm[8], qp[8];
+                cxr = cp + sy * xrow + (xl ? -1 : txe);
+                recon8<RECON>(prim, nc, cxr, 1, qm, qp);
+                if (xl) {
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) Qb.v[q][xrow][0] = qp[q];
+                }
+#pragma unroll
+                for (int q = 0; q < 8; ++q) xr_qm[q] = qm[q];
+            }
+            __syncthreads();
+            if (xr) {
+                double PL[8], Fh[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][xrow][txe];
+                face8<0>(prim, met, nc, cxr - 1, cxr, PL, xr_qm, gamma, Fh, nfb);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) Fb.v[q][xrow][txe] = Fh[q];
+            }
+            __syncthreads();
+            if (ycol) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) Qb.v[q][0][lane] = yb_qp[q];
+            }
+            __syncthreads();
+            if (ycol) {
+                double PL[8], Fh[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][tye][lane];
+                face8<1>(prim, met, nc, cyt - sy, cyt, PL, yt_qm, gamma, Fh, nfb);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) Fb.v[q][tye][lane] = Fh[q];
+            }
+            __syncthreads();
+        }
+    }
+    if (p.nfallback && nfb) atomicAdd(p.nfallback, (unsigned long long)nfb);
+}
+
+// ---- host side ------------------------------------------------------------------------------------------------
+namespace {
+
+struct Config { int ty, minb; };
+
+// GRX_TILE="<TY>x<MINB>" overrides the default tile (tuning knob; the compiled set is listed in dispatch()).
+Config pick_config() {
+    Config c = {7, 2};
+    if (const char* e = std::getenv("GRX_TILE")) {
+        int ty = 0, mb = 0;
+        if (std::sscanf(e, "%dx%d", &ty, &mb) == 2) { c.ty = ty; c.minb = mb; }
+    }
+    return c;
+}
+
+// z-chunking: enough CTAs to fill the machine a few times over, chunks long enough to amortise the two
+// one-sided plane steps at their ends.
+TileGeom make_tiles(const RhsParams& p, int ty, int slots) {
+    TileGeom tg;
+    tg.ntx = (p.n[0] + TX - 1) / TX;
+    tg.nty = (p.n[1] + ty - 1) / ty;
+    const long long inplane = (long long)tg.ntx * tg.nty * p.nbox;
+    int best = 1;
+    double best_eff = -1.0;
+    const int maxc = (p.n[2] + 7) / 8;
+    for (int nzc = 1; nzc <= maxc; ++nzc) {
+        const int tz = (p.n[2] + nzc - 1) / nzc;
+        const int real = (p.n[2] + tz - 1) / tz;
+        if (real != nzc) continue;
+        const double waves = (double)(inplane * nzc) / slots;
+        const double fill = waves / (double)(long long)(waves + 0.999999);
+        const double eff = fill * tz / (tz + 0.45);
+        if (eff > best_eff * 1.001) { best_eff = eff; best = nzc; }
+    }
+    tg.tz = (p.n[2] + best - 1) / best;
+    tg.nzc = (p.n[2] + tg.tz - 1) / tg.tz;
+    return tg;
+}
+
+template <int RECON, int TY, int MINB>
+cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
+    static int sms = 0;
+    if (sms == 0) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+    }
+    const size_t smem = 2 * sizeof(Exch<TY>);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(rhs_fused_kernel<RECON, TY, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const TileGeom tg = make_tiles(p, TY, sms * MINB);
+    const dim3 grid((unsigned)(tg.ntx * tg.nty * tg.nzc), p.nbox);
+    rhs_fused_kernel<RECON, TY, MINB><<<grid, (TY + 1) * 32, smem, st>>>(p, tg);
+    return cudaGetLastError();
+}
+
+template <int RECON>
+cudaError_t dispatch(const RhsParams& p, cudaStream_t st) {
+    const Config c = pick_config();
+    // compiled tiles: TY regular warps + 1 rim warp per CTA, MINB CTAs per SM (-> register budget)
+    if (c.ty == 7 && c.minb == 2) return launch_one<RECON, 7, 2>(p, st);     // 2 x 256 threads, 128 regs
+    if (c.ty == 11 && c.minb == 1) return launch_one<RECON, 11, 1>(p, st);   // 384 threads, 168 regs
+    if (c.ty == 5 && c.minb == 2) return launch_one<RECON, 5, 2>(p, st);     // 2 x 192 threads, 168 regs
+    if (c.ty == 15 && c.minb == 1) return launch_one<RECON, 15, 1>(p, st);   // 512 threads, 128 regs
+    if (c.ty == 7 && c.minb == 1) return launch_one<RECON, 7, 1>(p, st);     // 256 threads, 255 regs
+    return cudaErrorInvalidConfiguration;
+}
+
+}  // namespace
+
+cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st) {
+    if (recon == RECON_WENO5) return dispatch<RECON_WENO5>(p, st);
+    if (recon == RECON_MC) return dispatch<RECON_MC>(p, st);
+    return dispatch<RECON_MINMOD>(p, st);
+}
+
+}  // namespace grx

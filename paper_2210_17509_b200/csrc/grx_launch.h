@@ -1,0 +1,25 @@
+// grx_launch.h -- internal: host-side launchers implemented by the kernel translation units.
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include "grx_common.cuh"
+
+namespace grx {
+
+// grx_simple.cu: one thread per cell, every thread evaluates its own six faces (cross-check variant)
+cudaError_t launch_rhs_simple(const RhsParams& p, int recon, cudaStream_t st);
+// grx_fused.cu: the product kernel
+cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st);
+
+// grx_support.cu
+cudaError_t launch_prim2con(const double* prim, const double* met, long long nc, int nbox, double gamma, double* cons,
+                            cudaStream_t st);
+cudaError_t launch_con2prim(const double* cons, const double* met, long long nc, int nbox, double gamma, double* prim,
+                            unsigned long long* nfail, cudaStream_t st);
+cudaError_t launch_rk_axpy(const RhsParams& geom, double a, const double* x, double b, double dt, const double* rhs,
+                           double* y, cudaStream_t st);
+cudaError_t launch_selftest_math(const double* x, double* y, size_t n, cudaStream_t st);
+cudaError_t launch_dfma_peak(int iters, double* sink, double* flops_out, cudaStream_t st);
+
+}  // namespace grx

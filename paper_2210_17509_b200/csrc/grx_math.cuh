@@ -1,0 +1,427 @@
+// grx_math.cuh -- point-wise arithmetic of the Valencia GRMHD right-hand side (CUDA path).
+//
+// Everything here is per-point math: reconstruction of one cell (a2), face geometry (a1), one HLLE
+// face flux (a3-a6) and the geometric sources of one cell (a8-a9).  The kernels in grx_kernels.cu decide
+// who computes which point.  Citations are PAPER.md line numbers; R* are the readings in DESIGN.md.
+//
+// The formulas are algebraically those of the paper but arranged for the FP64 pipe of sm_100a: no IEEE
+// divisions (MUFU seed + one third-order correction, error < 1 ulp-ish, see rcp()/rsqrt()), a common
+// denominator for the WENO5 weights, a^2 = (b^2 + Gamma p)/(rho h*) for the fast speed, the sources in
+// their Eulerian-observer form.  All of these are rounding-level rearrangements (reading R26).
+//
+// The file also compiles as plain C++ (g++, tests/host_math_harness.cpp) so that the arithmetic can be
+// checked on a machine without a GPU; the host build is test infrastructure, never a product path.
+#pragma once
+
+#include <math.h>
+
+#if defined(__CUDACC__)
+#define GRX_HD __host__ __device__ __forceinline__
+#else
+#define GRX_HD inline
+#endif
+
+namespace grx {
+
+// ---- conventions (R4, R5) ----------------------------------------------------------------------------
+constexpr double WENO_EPS = 1e-26;       // Jiang-Shu epsilon
+constexpr double V2MAX    = 1.0 - 1e-4;  // admissibility bound on v^2 (W_max = 100)
+
+enum { RECON_MINMOD = 0, RECON_MC = 1, RECON_WENO5 = 2 };
+
+// ---- reciprocal, reciprocal square root, square root without the IEEE slow paths ----------------------
+// MUFU.RCP64H / MUFU.RSQ64H give ~20+ good bits; one third-order step brings the relative error to
+// ~1e-17 (grx_selftest_math + tests/test_gpu_parity.py::test_selftest_math measure it).  Arguments are
+// positive, normal numbers everywhere these are used (determinants, lapse, rho h*, 1 - v^2 a^2, ...).
+GRX_HD double rcp(double x) {
+#if defined(__CUDA_ARCH__)
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    double e2 = fma(e, e, e);
+    y = fma(y, e2, y);
+    e = fma(-x, y, 1.0);          // one Newton step on top: keeps 0.5 ulp-level accuracy even if the seed
+    return fma(y, e, y);          // is only 2^-14 good
+#else
+    return 1.0 / x;
+#endif
+}
+GRX_HD double rsqrt(double x) {
+#if defined(__CUDA_ARCH__)
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double t = x * y;
+    double h = fma(-t, y, 1.0);                 // 1 - x y^2
+    double p = fma(0.375, h, 0.5);
+    y = fma(y * h, p, y);                       // y (1 + h/2 + 3h^2/8)
+    t = x * y;
+    h = fma(-t, y, 1.0);
+    return fma(0.5 * y, h, y);                  // Newton step on top
+#else
+    return 1.0 / sqrt(x);
+#endif
+}
+// sqrt of a non-negative number (0 -> 0)
+GRX_HD double sqrt_nn(double x) {
+#if defined(__CUDA_ARCH__)
+    double s = x * rsqrt(x);
+    return (x > 0.0) ? s : 0.0;
+#else
+    return sqrt(x);
+#endif
+}
+
+// ---- a2: reconstruction of one cell ---------------------------------------------
+// (a,b,c,d,e) = (q_{i-2} .. q_{i+2});  qm = value at face i-1/2 from cell i, qp = value at face i+1/2.
+template <int RECON>
+GRX_HD void recon_cell(double a, double b, double c, double d, double e, double& qm, double& qp) {
+    if (RECON == RECON_WENO5) {
+        // Jiang-Shu WENO5 (ref [32]); written in first differences so that constant data is exact.
+        const double D1 = b - a, D2 = c - b, D3 = d - c, D4 = e - d;
+        const double t0 = D2 - D1, t1 = D3 - D2, t2 = D4 - D3;           // second differences
+        const double u0 = fma(3.0, D2, -D1);                              // a - 4b + 3c
+        const double u1 = D2 + D3;                                        // d - b
+        const double u2 = fma(-3.0, D3, D4);                              // 3c - 4d + e
+        // 4*beta_k = 13/3 t_k^2 + u_k^2  (the common factor 4 cancels in the weights; epsilon scaled alike)
+        const double k133 = 13.0 / 3.0;
+        const double B0 = fma(k133 * t0, t0, u0 * u0);
+        const double B1 = fma(k133 * t1, t1, u1 * u1);
+        const double B2 = fma(k133 * t2, t2, u2 * u2);
+        double e0 = B0 + 4.0 * WENO_EPS, e1 = B1 + 4.0 * WENO_EPS, e2 = B2 + 4.0 * WENO_EPS;
+        e0 *= e0; e1 *= e1; e2 *= e2;
+        // a_k = d_k / e_k  ->  multiply all three by e0 e1 e2 (common denominator, R26)
+        const double e01 = e0 * e1, e02 = e0 * e2, e12 = e1 * e2;
+        const double w1 = 6.0 * e02;
+        // plus side: weights (1,6,3)/10 on (e12, e02, e01)
+        const double wp2 = 3.0 * e01;
+        const double Sp = e12 + w1 + wp2;
+        // 6 p_k - 6 c in differences
+        const double pp0 = fma(5.0, D2, -2.0 * D1), pp1 = fma(2.0, D3, D2), pp2 = fma(4.0, D3, -D4);
+        const double Np = fma(wp2, pp2, fma(w1, pp1, e12 * pp0));
+        // minus side: mirrored stencil, weights (1,6,3)/10 on (e01, e02, e12)
+        const double wm2 = 3.0 * e12;
+        const double Sm = e01 + w1 + wm2;
+        const double pm0 = fma(-5.0, D3, 2.0 * D4), pm1 = -fma(2.0, D2, D3), pm2 = fma(-4.0, D2, D1);
+        const double Nm = fma(wm2, pm2, fma(w1, pm1, e01 * pm0));
+        const double r = rcp(Sp * Sm) * (1.0 / 6.0);
+        qp = fma(Np, Sm * r, c);
+        qm = fma(Nm, Sp * r, c);
+    } else {
+        const double dm = c - b, dp = d - c;
+        double sigma = 0.0;
+        if (dm * dp > 0.0) {
+            if (RECON == RECON_MC) {
+                // monotonised central: sign * min(2|dm|, 2|dp|, |dm+dp|/2)
+                const double m = fmin(fmin(2.0 * fabs(dm), 2.0 * fabs(dp)), 0.5 * fabs(dm + dp));
+                sigma = (dm > 0.0) ? m : -m;
+            } else {
+                sigma = (fabs(dm) < fabs(dp)) ? dm : dp;   // minmod (l.255)
+            }
+        }
+        qm = fma(-0.5, sigma, c);
+        qp = fma(0.5, sigma, c);
+    }
+}
+
+// ---- a1: geometry of one face (l.130; R6, R7) -----------------------------------------------------------
+struct FaceGeom {
+    double alp;            // lapse
+    double beta[3];        // shift beta^i
+    double g[6];           // gamma_ij: xx xy xz yy yz zz
+    double sg;             // sqrt(det gamma)
+    double gdd;            // gamma^{dd} for the sweep direction
+};
+// alp, beta, g already hold the two-point averages; completes sg and gdd.
+template <int D>
+GRX_HD void face_geom_complete(FaceGeom& m) {
+    const double gxx = m.g[0], gxy = m.g[1], gxz = m.g[2], gyy = m.g[3], gyz = m.g[4], gzz = m.g[5];
+    const double cxx = fma(gyy, gzz, -gyz * gyz);
+    const double cxy = fma(gxz, gyz, -gxy * gzz);
+    const double cxz = fma(gxy, gyz, -gxz * gyy);
+    const double det = fma(gxx, cxx, fma(gxy, cxy, gxz * cxz));
+    const double rs = rsqrt(det);
+    m.sg = det * rs;
+    const double cdd = (D == 0) ? cxx : (D == 1) ? fma(gxx, gzz, -gxz * gxz) : fma(gxx, gyy, -gxy * gxy);
+    m.gdd = cdd * (rs * rs);
+}
+
+// ---- a3-a5: one side of a face: admissibility, conserved state, flux, fast speeds -------------------------
+// P: reconstructed primitives of this side; cen[q * nc]: centre values of its donor cell, read only if the
+// side takes the first-order fallback (R5).
+// Returns U (Eqs. 6-9, l.88-94), F^D (Eq. 12, l.108) and the two characteristic speeds (R8).
+template <int D>
+GRX_HD void side_state(const double Pin[8], const double* __restrict__ cen, long long nc, const FaceGeom& m,
+                       double gamma, double U[8], double F[8], double& lam_m, double& lam_p, unsigned& nfallback) {
+    double rho = Pin[0], vx = Pin[1], vy = Pin[2], vz = Pin[3], eps = Pin[4];
+    double Bx = Pin[5], By = Pin[6], Bz = Pin[7];
+    const double gxx = m.g[0], gxy = m.g[1], gxz = m.g[2], gyy = m.g[3], gyz = m.g[4], gzz = m.g[5];
+    double vlx = fma(gxx, vx, fma(gxy, vy, gxz * vz));      // v_i = gamma_ij v^j
+    double vly = fma(gxy, vx, fma(gyy, vy, gyz * vz));
+    double vlz = fma(gxz, vx, fma(gyz, vy, gzz * vz));
+    double v2 = fma(vlx, vx, fma(vly, vy, vlz * vz));
+    if (!(rho > 0.0 && eps > 0.0 && v2 < V2MAX)) {          // R5; NaN fails the test
+        rho = cen[0]; vx = cen[nc]; vy = cen[2 * nc]; vz = cen[3 * nc]; eps = cen[4 * nc];
+        Bx = cen[5 * nc]; By = cen[6 * nc]; Bz = cen[7 * nc];
+        vlx = fma(gxx, vx, fma(gxy, vy, gxz * vz));
+        vly = fma(gxy, vx, fma(gyy, vy, gyz * vz));
+        vlz = fma(gxz, vx, fma(gyz, vy, gzz * vz));
+        v2 = fma(vlx, vx, fma(vly, vy, vlz * vz));
+        ++nfallback;
+    }
+    const double iW2 = 1.0 - v2;                             // 1/W^2
+    const double W = rsqrt(iW2);                             // l.98
+    const double iW = W * iW2;
+    const double W2 = W * W;
+    const double Blx = fma(gxx, Bx, fma(gxy, By, gxz * Bz));
+    const double Bly = fma(gxy, Bx, fma(gyy, By, gyz * Bz));
+    const double Blz = fma(gxz, Bx, fma(gyz, By, gzz * Bz));
+    const double B2 = fma(Blx, Bx, fma(Bly, By, Blz * Bz));
+    const double Bv = fma(Bx, vlx, fma(By, vly, Bz * vlz));
+    const double ab0 = W * Bv;                               // alpha b^0
+    const double b2 = fma(B2, iW2, Bv * Bv);                 // b^2
+    const double blx = fma(Blx, iW, ab0 * vlx);              // b_i
+    const double bly = fma(Bly, iW, ab0 * vly);
+    const double blz = fma(Blz, iW, ab0 * vlz);
+    const double rhoeps = rho * eps;
+    const double p = (gamma - 1.0) * rhoeps;                 // l.138
+    const double rhoh = fma(gamma, rhoeps, rho);             // rho (1 + eps) + p
+    const double rhohs = rhoh + b2;                          // rho h*
+    const double Ps = fma(0.5, b2, p);                       // P*
+    const double X = rhohs * W2;
+    const double sg = m.sg;
+    const double Dd = sg * rho * W;                          // Eq. (6)
+    const double Sx = sg * fma(X, vlx, -ab0 * blx);          // Eq. (7)
+    const double Sy = sg * fma(X, vly, -ab0 * bly);
+    const double Sz = sg * fma(X, vlz, -ab0 * blz);
+    const double tau = fma(sg, fma(-ab0, ab0, X - Ps), -Dd); // Eq. (8)
+    const double cBx = sg * Bx, cBy = sg * By, cBz = sg * Bz;  // Eq. (9)
+    U[0] = Dd; U[1] = Sx; U[2] = Sy; U[3] = Sz; U[4] = tau; U[5] = cBx; U[6] = cBy; U[7] = cBz;
+    // flux, Eq. (12): vtilde^i = v^i - beta^i/alpha (l.114); everything carries one factor alpha
+    const double alp = m.alp;
+    const double avx = fma(alp, vx, -m.beta[0]);             // alpha vtilde^i
+    const double avy = fma(alp, vy, -m.beta[1]);
+    const double avz = fma(alp, vz, -m.beta[2]);
+    const double vd = (D == 0) ? vx : (D == 1) ? vy : vz;
+    const double avd = (D == 0) ? avx : (D == 1) ? avy : avz;
+    const double cBd = (D == 0) ? cBx : (D == 1) ? cBy : cBz;
+    const double aBdW = alp * cBd * iW;                      // alpha calB^d / W
+    const double asgPs = alp * sg * Ps;
+    F[0] = Dd * avd;
+    F[1] = fma(Sx, avd, -blx * aBdW);
+    F[2] = fma(Sy, avd, -bly * aBdW);
+    F[3] = fma(Sz, avd, -blz * aBdW);
+    F[1 + D] += asgPs;
+    F[4] = fma(tau, avd, fma(asgPs, vd, -ab0 * aBdW));
+    F[5] = fma(cBx, avd, -cBd * avx);
+    F[6] = fma(cBy, avd, -cBd * avy);
+    F[7] = fma(cBz, avd, -cBd * avz);
+    F[5 + D] = 0.0;
+    // fast-magnetosonic speeds (R8): a^2 = cs^2 + vA^2 - cs^2 vA^2 = (b^2 + Gamma p)/(rho h*)
+    const double gp = gamma * p;
+    const double irhohs = rcp(rhohs);
+    const double a2 = (b2 + gp) * irhohs;
+    const double oma2 = (rhoh - gp) * irhohs;                // 1 - a^2
+    const double den = fma(-v2, a2, 1.0);                    // 1 - v^2 a^2
+    const double iden = rcp(den);
+    const double disc = a2 * iW2 * fma(m.gdd, den, -vd * vd * oma2);
+    const double root = sqrt_nn(fmax(disc, 0.0));
+    const double c0 = vd * oma2;
+    const double ai = alp * iden;
+    const double bd = m.beta[D];
+    lam_p = fma(ai, c0 + root, -bd);
+    lam_m = fma(ai, c0 - root, -bd);
+}
+
+// ---- a6: HLLE flux of one face (l.131; R9) -----------------------------------------------------------------
+// m holds the averaged alp, beta, g on entry; cenL/cenR point at field 0 of the two donor cells (field stride nc).
+template <int D>
+GRX_HD void face_flux(FaceGeom& m, const double PL[8], const double PR[8], const double* __restrict__ cenL,
+                      const double* __restrict__ cenR, long long nc, double gamma, double Fh[8], unsigned& nfallback) {
+    face_geom_complete<D>(m);
+    double UL[8], FL[8], UR[8], FR[8], lmL, lpL, lmR, lpR;
+    side_state<D>(PL, cenL, nc, m, gamma, UL, FL, lmL, lpL, nfallback);
+    side_state<D>(PR, cenR, nc, m, gamma, UR, FR, lmR, lpR, nfallback);
+    const double lm = fmin(0.0, fmin(lmL, lmR));
+    const double lp = fmax(0.0, fmax(lpL, lpR));
+    const double idl = rcp(lp - lm);
+    const double cL = lp * idl, cR = -lm * idl, cU = lp * lm * idl;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) Fh[c] = fma(cL, FL[c], fma(cR, FR[c], cU * (UR[c] - UL[c])));
+}
+
+// ---- a8: 4th-order centred first derivative, grouped so that a constant differentiates to exactly 0 (R12) ---
+GRX_HD double d4(double mm2, double mm1, double mp1, double mp2, double inv12dx) {
+    return fma(8.0, mp1 - mm1, -(mp2 - mm2)) * inv12dx;
+}
+
+// ---- a9: geometric sources of one cell, Eq. (13) (l.112) in 3+1 form (R12-R14) -------------------------------
+// With the Eulerian-observer quantities  E = rho h* W^2 - P* - (alpha b^0)^2,  S_k = rho h* W^2 v_k - alpha b^0 b_k,
+// S^{kl} = rho h* W^2 v^k v^l + P* gamma^{kl} - bb^k bb^l  (bb^k = B^k/W + alpha b^0 v^k)  Eq. (13) becomes
+//   S_{S_j} = sqrt(gamma) [ alpha/2 S^{kl} d_j gamma_kl + S_k d_j beta^k - E d_j alpha ],
+//   S_tau   = sqrt(gamma) [ alpha K_kl S^{kl} - S^k d_k alpha ],
+// which is term by term the same as the T^{mu nu} form the oracle evaluates.
+// P: cell-centre primitives; met: the 10 metric fields at the centre; K: K_ij; dm[j][f] = d_j of metric field f.
+GRX_HD void sources_point(const double P[8], const double met[10], const double K[6], const double dm[3][10],
+                          double gamma, double& SSx, double& SSy, double& SSz, double& Stau) {
+    const double rho = P[0], vx = P[1], vy = P[2], vz = P[3], eps = P[4], Bx = P[5], By = P[6], Bz = P[7];
+    const double alp = met[0];
+    const double gxx = met[4], gxy = met[5], gxz = met[6], gyy = met[7], gyz = met[8], gzz = met[9];
+    const double cxx = fma(gyy, gzz, -gyz * gyz);
+    const double cxy = fma(gxz, gyz, -gxy * gzz);
+    const double cxz = fma(gxy, gyz, -gxz * gyy);
+    const double cyy = fma(gxx, gzz, -gxz * gxz);
+    const double cyz = fma(gxy, gxz, -gxx * gyz);
+    const double czz = fma(gxx, gyy, -gxy * gxy);
+    const double det = fma(gxx, cxx, fma(gxy, cxy, gxz * cxz));
+    const double rs = rsqrt(det);
+    const double sg = det * rs, idet = rs * rs;
+    const double vlx = fma(gxx, vx, fma(gxy, vy, gxz * vz));
+    const double vly = fma(gxy, vx, fma(gyy, vy, gyz * vz));
+    const double vlz = fma(gxz, vx, fma(gyz, vy, gzz * vz));
+    const double v2 = fma(vlx, vx, fma(vly, vy, vlz * vz));
+    const double iW2 = 1.0 - v2;
+    const double W = rsqrt(iW2), iW = W * iW2, W2 = W * W;
+    const double Blx = fma(gxx, Bx, fma(gxy, By, gxz * Bz));
+    const double Bly = fma(gxy, Bx, fma(gyy, By, gyz * Bz));
+    const double Blz = fma(gxz, Bx, fma(gyz, By, gzz * Bz));
+    const double B2 = fma(Blx, Bx, fma(Bly, By, Blz * Bz));
+    const double Bv = fma(Bx, vlx, fma(By, vly, Bz * vlz));
+    const double ab0 = W * Bv;
+    const double b2 = fma(B2, iW2, Bv * Bv);
+    const double rhoeps = rho * eps;
+    const double p = (gamma - 1.0) * rhoeps;
+    const double rhohs = fma(gamma, rhoeps, rho) + b2;
+    const double Ps = fma(0.5, b2, p);
+    const double X = rhohs * W2;
+    const double E = fma(-ab0, ab0, X - Ps);
+    // bb^k (upper) and bb_k (lower), momentum density S_k (lower) and S^k (upper)
+    const double bux = fma(Bx, iW, ab0 * vx), buy = fma(By, iW, ab0 * vy), buz = fma(Bz, iW, ab0 * vz);
+    const double blx = fma(Blx, iW, ab0 * vlx), bly = fma(Bly, iW, ab0 * vly), blz = fma(Blz, iW, ab0 * vlz);
+    const double Slx = fma(X, vlx, -ab0 * blx), Sly = fma(X, vly, -ab0 * bly), Slz = fma(X, vlz, -ab0 * blz);
+    const double Sux = fma(X, vx, -ab0 * bux), Suy = fma(X, vy, -ab0 * buy), Suz = fma(X, vz, -ab0 * buz);
+    // spatial stress S^{kl}
+    const double Pi = Ps * idet;   // P* gamma^{kl} = P*/det * cofactor
+    const double Xvx = X * vx, Xvy = X * vy, Xvz = X * vz;
+    const double Sxx = fma(Xvx, vx, fma(Pi, cxx, -bux * bux));
+    const double Sxy = fma(Xvx, vy, fma(Pi, cxy, -bux * buy));
+    const double Sxz = fma(Xvx, vz, fma(Pi, cxz, -bux * buz));
+    const double Syy = fma(Xvy, vy, fma(Pi, cyy, -buy * buy));
+    const double Syz = fma(Xvy, vz, fma(Pi, cyz, -buy * buz));
+    const double Szz = fma(Xvz, vz, fma(Pi, czz, -buz * buz));
+    const double ha = 0.5 * alp;
+    double SS[3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const double* d = dm[j];
+        // alpha/2 S^{kl} d_j gamma_kl  (off-diagonal terms count twice)
+        const double sdg = fma(Sxx, d[4], fma(Syy, d[7], Szz * d[9])) * ha +
+                           alp * fma(Sxy, d[5], fma(Sxz, d[6], Syz * d[8]));
+        const double sdb = fma(Slx, d[1], fma(Sly, d[2], Slz * d[3]));
+        SS[j] = sg * (sdg + fma(-E, d[0], sdb));
+    }
+    SSx = SS[0]; SSy = SS[1]; SSz = SS[2];
+    const double KS = fma(K[0], Sxx, fma(K[3], Syy, K[5] * Szz)) + 2.0 * fma(K[1], Sxy, fma(K[2], Sxz, K[4] * Syz));
+    const double Sda = fma(Sux, dm[0][0], fma(Suy, dm[1][0], Suz * dm[2][0]));
+    Stau = sg * fma(alp, KS, -Sda);
+}
+
+// ---- prim2con at one point with the full metric given (Eqs. 6-9) ----------------------------------------------
+GRX_HD void prim2con_point(const double P[8], const double met[10], double gamma, double U[8]) {
+    const double rho = P[0], vx = P[1], vy = P[2], vz = P[3], eps = P[4], Bx = P[5], By = P[6], Bz = P[7];
+    const double gxx = met[4], gxy = met[5], gxz = met[6], gyy = met[7], gyz = met[8], gzz = met[9];
+    const double cxx = fma(gyy, gzz, -gyz * gyz);
+    const double cxy = fma(gxz, gyz, -gxy * gzz);
+    const double cxz = fma(gxy, gyz, -gxz * gyy);
+    const double det = fma(gxx, cxx, fma(gxy, cxy, gxz * cxz));
+    const double sg = sqrt(det);
+    const double vlx = fma(gxx, vx, fma(gxy, vy, gxz * vz));
+    const double vly = fma(gxy, vx, fma(gyy, vy, gyz * vz));
+    const double vlz = fma(gxz, vx, fma(gyz, vy, gzz * vz));
+    const double v2 = fma(vlx, vx, fma(vly, vy, vlz * vz));
+    const double iW2 = 1.0 - v2;
+    const double W = 1.0 / sqrt(iW2), iW = W * iW2, W2 = W * W;
+    const double Blx = fma(gxx, Bx, fma(gxy, By, gxz * Bz));
+    const double Bly = fma(gxy, Bx, fma(gyy, By, gyz * Bz));
+    const double Blz = fma(gxz, Bx, fma(gyz, By, gzz * Bz));
+    const double B2 = fma(Blx, Bx, fma(Bly, By, Blz * Bz));
+    const double Bv = fma(Bx, vlx, fma(By, vly, Bz * vlz));
+    const double ab0 = W * Bv;
+    const double b2 = fma(B2, iW2, Bv * Bv);
+    const double rhoeps = rho * eps;
+    const double p = (gamma - 1.0) * rhoeps;
+    const double rhohs = fma(gamma, rhoeps, rho) + b2;
+    const double Ps = fma(0.5, b2, p);
+    const double X = rhohs * W2;
+    const double Dd = sg * rho * W;
+    U[0] = Dd;
+    U[1] = sg * fma(X, vlx, -ab0 * fma(Blx, iW, ab0 * vlx));
+    U[2] = sg * fma(X, vly, -ab0 * fma(Bly, iW, ab0 * vly));
+    U[3] = sg * fma(X, vlz, -ab0 * fma(Blz, iW, ab0 * vlz));
+    U[4] = fma(sg, fma(-ab0, ab0, X - Ps), -Dd);
+    U[5] = sg * Bx; U[6] = sg * By; U[7] = sg * Bz;
+}
+
+// ---- support (R22): Gamma-law con2prim at one point, Newton on z = rho h W^2 with a bracket -----------------
+// Returns 0 on convergence, 1 otherwise.
+GRX_HD int con2prim_point(const double U[8], const double met[10], double gamma, double P[8]) {
+    const double gxx = met[4], gxy = met[5], gxz = met[6], gyy = met[7], gyz = met[8], gzz = met[9];
+    const double cxx = fma(gyy, gzz, -gyz * gyz);
+    const double cxy = fma(gxz, gyz, -gxy * gzz);
+    const double cxz = fma(gxy, gyz, -gxz * gyy);
+    const double cyy = fma(gxx, gzz, -gxz * gxz);
+    const double cyz = fma(gxy, gxz, -gxx * gyz);
+    const double czz = fma(gxx, gyy, -gxy * gxy);
+    const double det = fma(gxx, cxx, fma(gxy, cxy, gxz * cxz));
+    const double isg = 1.0 / sqrt(det), idet = 1.0 / det;
+    const double Dd = U[0] * isg, tau = U[4] * isg;
+    const double Slx = U[1] * isg, Sly = U[2] * isg, Slz = U[3] * isg;
+    const double Bx = U[5] * isg, By = U[6] * isg, Bz = U[7] * isg;
+    const double Sux = (cxx * Slx + cxy * Sly + cxz * Slz) * idet;
+    const double Suy = (cxy * Slx + cyy * Sly + cyz * Slz) * idet;
+    const double Suz = (cxz * Slx + cyz * Sly + czz * Slz) * idet;
+    const double Blx = gxx * Bx + gxy * By + gxz * Bz;
+    const double Bly = gxy * Bx + gyy * By + gyz * Bz;
+    const double Blz = gxz * Bx + gyz * By + gzz * Bz;
+    const double S2 = Slx * Sux + Sly * Suy + Slz * Suz;
+    const double B2 = Blx * Bx + Bly * By + Blz * Bz;
+    const double SB = Slx * Bx + Sly * By + Slz * Bz;
+    const double E = tau + Dd;
+    const double SB2 = SB * SB;
+    double W = 1.0, rho = Dd, p = 0.0;
+    auto eval = [&](double z) {
+        double v2 = (S2 * z * z + SB2 * (B2 + 2.0 * z)) / ((z + B2) * (z + B2) * z * z);
+        if (v2 > 1.0 - 1e-15) v2 = 1.0 - 1e-15;
+        W = 1.0 / sqrt(1.0 - v2);
+        rho = Dd / W;
+        p = (gamma - 1.0) / gamma * (z / (W * W) - rho);
+        return z + B2 - p - B2 / (2.0 * W * W) - SB2 / (2.0 * z * z) - E;
+    };
+    double zhi = fmax(2.0 * (E + 1.0), 1.0);
+    for (int it = 0; it < 200 && eval(zhi) < 0.0; ++it) zhi *= 2.0;
+    double zlo = zhi;
+    for (int it = 0; it < 400 && eval(zlo) > 0.0; ++it) zlo *= 0.5;
+    double z = 0.5 * (zlo + zhi);
+    int status = 1;
+    for (int it = 0; it < 200; ++it) {
+        const double f = eval(z);
+        if (f > 0.0) zhi = z; else zlo = z;
+        const double h = 1e-6 * z;
+        const double fp = (eval(z + h) - eval(z - h)) / (2.0 * h);
+        double zn = z - f / fp;
+        if (!(zn > zlo && zn < zhi)) zn = 0.5 * (zlo + zhi);
+        const double dz = fabs(zn - z);
+        z = zn;
+        if (dz < 1e-14 * z) { status = 0; break; }
+    }
+    eval(z);
+    P[0] = rho;
+    const double iz = 1.0 / z, izb = 1.0 / (z + B2);
+    P[1] = (Sux + SB * Bx * iz) * izb;
+    P[2] = (Suy + SB * By * iz) * izb;
+    P[3] = (Suz + SB * Bz * iz) * izb;
+    P[4] = p / ((gamma - 1.0) * rho);
+    P[5] = Bx; P[6] = By; P[7] = Bz;
+    return status;
+}
+
+}  // namespace grx

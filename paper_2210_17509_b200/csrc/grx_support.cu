@@ -1,0 +1,130 @@
+// grx_support.cu -- small kernels around the hot path: prim2con (Eqs. 6-9), the support
+// con2prim and RK update (R21/R22), the accuracy self-test of rcp/rsqrt and the DFMA peak micro-benchmark.
+#include "grx_launch.h"
+
+namespace grx {
+
+__global__ void __launch_bounds__(256) prim2con_kernel(const double* __restrict__ prim, const double* __restrict__ met,
+                                                       long long nc, double gamma, double* __restrict__ cons) {
+    const long long c0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c0 >= nc) return;
+    const long long box = blockIdx.y;
+    const double* pb = prim + box * 8 * nc;
+    const double* mb = met + box * 10 * nc;
+    double* cb = cons + box * 8 * nc;
+    double P[8], m[10], U[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) P[q] = pb[q * nc + c0];
+#pragma unroll
+    for (int f = 0; f < 10; ++f) m[f] = mb[f * nc + c0];
+    prim2con_point(P, m, gamma, U);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) cb[q * nc + c0] = U[q];
+}
+
+__global__ void __launch_bounds__(128) con2prim_kernel(const double* __restrict__ cons, const double* __restrict__ met,
+                                                       long long nc, double gamma, double* __restrict__ prim,
+                                                       unsigned long long* nfail) {
+    const long long c0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c0 >= nc) return;
+    const long long box = blockIdx.y;
+    const double* cb = cons + box * 8 * nc;
+    const double* mb = met + box * 10 * nc;
+    double* pb = prim + box * 8 * nc;
+    double P[8], m[10], U[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) U[q] = cb[q * nc + c0];
+#pragma unroll
+    for (int f = 0; f < 10; ++f) m[f] = mb[f * nc + c0];
+    const int bad = con2prim_point(U, m, gamma, P);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) pb[q * nc + c0] = P[q];
+    if (bad && nfail) atomicAdd(nfail, 1ULL);
+}
+
+__global__ void __launch_bounds__(128) rk_axpy_kernel(const __grid_constant__ RhsParams p, double a,
+                                                      const double* __restrict__ x, double b, double dt,
+                                                      const double* __restrict__ rhs, double* y) {
+    const int nxb = (p.n[0] + 127) / 128;
+    const int i = (blockIdx.x % nxb) * 128 + threadIdx.x;
+    const int row = blockIdx.x / nxb;
+    const int j = row % p.n[1], k = row / p.n[1];
+    if (i >= p.n[0]) return;
+    const long long base = (long long)blockIdx.y * 8 * p.nc + (i + p.g) + p.stride[1] * (j + p.g) + p.stride[2] * (k + p.g);
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const long long o = base + c * p.nc;
+        y[o] = a * x[o] + b * (y[o] + dt * rhs[o]);
+    }
+}
+
+__global__ void selftest_math_kernel(const double* __restrict__ x, double* __restrict__ y, size_t n) {
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const double v = x[t];
+    y[t] = rcp(v);
+    y[n + t] = rsqrt(v);
+    y[2 * n + t] = sqrt_nn(v);
+}
+
+// 8 independent FMA chains per thread; every lane of the FP64 pipe busy, nothing else going on.
+constexpr int DFMA_CHAINS = 8;
+constexpr int DFMA_THREADS = 256;
+__global__ void __launch_bounds__(DFMA_THREADS) dfma_peak_kernel(int iters, double* sink) {
+    double a[DFMA_CHAINS];
+    const double m = 1.0 + 1e-9 * threadIdx.x, c = 1e-12 * blockIdx.x;
+#pragma unroll
+    for (int q = 0; q < DFMA_CHAINS; ++q) a[q] = 0.1 * (q + 1);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+#pragma unroll
+            for (int q = 0; q < DFMA_CHAINS; ++q) a[q] = fma(a[q], m, c);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < DFMA_CHAINS; ++q) s += a[q];
+    if (s == 1.2345678) *sink = s;   // keeps the chains alive without a store in the common case
+}
+
+cudaError_t launch_prim2con(const double* prim, const double* met, long long nc, int nbox, double gamma, double* cons,
+                            cudaStream_t st) {
+    const dim3 grid((unsigned)((nc + 255) / 256), nbox);
+    prim2con_kernel<<<grid, 256, 0, st>>>(prim, met, nc, gamma, cons);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_con2prim(const double* cons, const double* met, long long nc, int nbox, double gamma, double* prim,
+                            unsigned long long* nfail, cudaStream_t st) {
+    const dim3 grid((unsigned)((nc + 127) / 128), nbox);
+    con2prim_kernel<<<grid, 128, 0, st>>>(cons, met, nc, gamma, prim, nfail);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rk_axpy(const RhsParams& p, double a, const double* x, double b, double dt, const double* rhs,
+                           double* y, cudaStream_t st) {
+    const dim3 grid((unsigned)((p.n[0] + 127) / 128) * (unsigned)p.n[1] * (unsigned)p.n[2], p.nbox);
+    rk_axpy_kernel<<<grid, 128, 0, st>>>(p, a, x, b, dt, rhs, y);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_selftest_math(const double* x, double* y, size_t n, cudaStream_t st) {
+    if (n == 0) return cudaSuccess;
+    selftest_math_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(x, y, n);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_dfma_peak(int iters, double* sink, double* flops_out, cudaStream_t st) {
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    const int blocks = sms * 4;   // 4 x 256 threads per SM: 8 warps per scheduler
+    dfma_peak_kernel<<<blocks, DFMA_THREADS, 0, st>>>(iters, sink);
+    if (flops_out) *flops_out = 2.0 * 4.0 * DFMA_CHAINS * (double)iters * DFMA_THREADS * (double)blocks;
+    return cudaGetLastError();
+}
+
+}  // namespace grx

@@ -1,0 +1,200 @@
+"""Thin binding of the C-ABI library (include/grx.h): argument marshalling only.
+
+Every function takes torch CUDA float64 tensors (device memory and streams are PyTorch's; all
+arithmetic happens in libgrx.so) in the library's layout [nbox, nfield, Nz, Ny, Nx], x fastest.
+There is no CPU path: `lib()` raises if libgrx.so has not been built, and every call raises GrxError on a
+non-zero return code.
+
+    from paper_2210_17509_b200 import grx
+    out = grx.valencia_rhs(prim, metric, K, dx, nghost=3, recon="weno5", gamma=5/3)
+"""
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgrx.so")
+
+RECON = {"minmod": 0, "mc": 1, "weno5": 2}
+VARIANT = {"fused": 0, "simple": 1}
+EXPORTS = (
+    "grx_valencia_rhs", "grx_valencia_rhs_host", "grx_host_workspace_bytes", "grx_prim2con", "grx_con2prim", "grx_rk_axpy", "grx_debug_set_fallback_counter",
+    "grx_set_variant", "grx_selftest_math", "grx_dfma_peak_launch", "grx_last_error", "grx_version",
+    "grx_weno_eps", "grx_v2max",
+)
+
+
+class GrxError(RuntimeError):
+    pass
+
+
+class grx_grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("nbox", C.c_int)]
+
+
+_lib = None
+
+
+def lib():
+    """Loads libgrx.so (built by `python -m paper_2210_17509_b200.build`); raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise GrxError(f"{LIB_PATH} not found: build it with `python -m paper_2210_17509_b200.build` "
+                           "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, dbl, i, sz = C.c_void_p, C.c_double, C.c_int, C.c_size_t
+        gp = C.POINTER(grx_grid)
+        d3 = C.POINTER(C.c_double)
+        L.grx_valencia_rhs.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, vp]
+        L.grx_valencia_rhs_host.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, vp, sz, vp]
+        L.grx_host_workspace_bytes.argtypes = [gp, i]
+        L.grx_prim2con.argtypes = [gp, vp, vp, i, dbl, vp, vp]
+        L.grx_con2prim.argtypes = [gp, vp, vp, i, dbl, vp, vp, vp]
+        L.grx_rk_axpy.argtypes = [gp, i, dbl, vp, dbl, dbl, vp, vp, vp]
+        L.grx_debug_set_fallback_counter.argtypes = [vp]
+        L.grx_set_variant.argtypes = [i]
+        L.grx_selftest_math.argtypes = [vp, vp, sz, vp]
+        L.grx_dfma_peak_launch.argtypes = [i, vp, d3, vp]
+        for name in EXPORTS:
+            getattr(L, name).restype = C.c_int
+        L.grx_host_workspace_bytes.restype = sz
+        L.grx_last_error.restype = C.c_char_p
+        L.grx_weno_eps.restype = dbl
+        L.grx_v2max.restype = dbl
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise GrxError(f"grx error {rc}: {lib().grx_last_error().decode()}")
+
+
+def _stream(stream=None):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _dev(t, nfield=None):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise GrxError("expected a contiguous CUDA float64 tensor")
+    if nfield is not None and (t.dim() != 5 or t.shape[1] != nfield):
+        raise GrxError(f"expected shape [nbox, {nfield}, Nz, Ny, Nx], got {tuple(t.shape)}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _grid(t, nghost):
+    nbox, _, Nz, Ny, Nx = t.shape
+    return grx_grid(Nx - 2 * nghost, Ny - 2 * nghost, Nz - 2 * nghost, nbox)
+
+
+def valencia_rhs(prim, metric, K, dx, nghost, recon, gamma, out=None, stream=None):
+    """grx_valencia_rhs: d/dt of (D, S_i, tau, calB^i) on the interior cells (asynchronous on the stream).
+    `out` (same shape as prim) is allocated if not given; its ghost cells are left untouched."""
+    import torch
+    if out is None:
+        out = torch.empty_like(prim)
+    g = _grid(prim, nghost)
+    if metric.shape[0] != prim.shape[0] or K.shape[0] != prim.shape[0] or metric.shape[2:] != prim.shape[2:] \
+            or K.shape[2:] != prim.shape[2:] or out.shape != prim.shape:
+        raise GrxError("prim, metric, K, out must share nbox and the spatial shape")
+    r = RECON[recon] if isinstance(recon, str) else int(recon)
+    dxa = (C.c_double * 3)(*[float(v) for v in dx])
+    _check(lib().grx_valencia_rhs(C.byref(g), _dev(prim, 8), _dev(metric, 10), _dev(K, 6), dxa, int(nghost), r,
+                                  float(gamma), _dev(out, 8), _stream(stream)))
+    return out
+
+
+def host_workspace_bytes(shape, nghost):
+    nbox, _, Nz, Ny, Nx = shape
+    g = grx_grid(Nx - 2 * nghost, Ny - 2 * nghost, Nz - 2 * nghost, nbox)
+    return lib().grx_host_workspace_bytes(C.byref(g), int(nghost))
+
+
+def valencia_rhs_host(prim, metric, K, dx, nghost, recon, gamma, out, workspace, stream=None):
+    """grx_valencia_rhs_host: prim/metric/K/out are HOST tensors (float64, contiguous, ideally pinned);
+    `workspace` is a CUDA tensor of at least host_workspace_bytes(prim.shape, nghost) bytes.  Asynchronous:
+    `out` is valid after the stream is synchronised."""
+    import torch
+    for t in (prim, metric, K, out):
+        if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise GrxError("expected contiguous host float64 tensors")
+    if not workspace.is_cuda:
+        raise GrxError("workspace must be a CUDA tensor")
+    g = _grid(prim, nghost)
+    r = RECON[recon] if isinstance(recon, str) else int(recon)
+    dxa = (C.c_double * 3)(*[float(v) for v in dx])
+    _check(lib().grx_valencia_rhs_host(C.byref(g), C.c_void_p(prim.data_ptr()), C.c_void_p(metric.data_ptr()),
+                                       C.c_void_p(K.data_ptr()), dxa, int(nghost), r, float(gamma),
+                                       C.c_void_p(out.data_ptr()), C.c_void_p(workspace.data_ptr()),
+                                       workspace.numel() * workspace.element_size(), _stream(stream)))
+    return out
+
+
+def prim2con(prim, metric, nghost, gamma, out=None, stream=None):
+    import torch
+    if out is None:
+        out = torch.empty_like(prim)
+    g = _grid(prim, nghost)
+    _check(lib().grx_prim2con(C.byref(g), _dev(prim, 8), _dev(metric, 10), int(nghost), float(gamma), _dev(out, 8),
+                              _stream(stream)))
+    return out
+
+
+def con2prim(cons, metric, nghost, gamma, out=None, nfail=None, stream=None):
+    """Support code (R22).  nfail: optional CUDA int64 tensor of one element, incremented per failed cell."""
+    import torch
+    if out is None:
+        out = torch.empty_like(cons)
+    g = _grid(cons, nghost)
+    nf = C.c_void_p(nfail.data_ptr()) if nfail is not None else C.c_void_p(0)
+    _check(lib().grx_con2prim(C.byref(g), _dev(cons, 8), _dev(metric, 10), int(nghost), float(gamma), _dev(out, 8), nf,
+                              _stream(stream)))
+    return out
+
+
+def rk_axpy(a, x, b, dt, rhs, y, nghost, stream=None):
+    """y[int] = a*x[int] + b*(y[int] + dt*rhs[int])  (support code, R21)."""
+    g = _grid(x, nghost)
+    _check(lib().grx_rk_axpy(C.byref(g), int(nghost), float(a), _dev(x, 8), float(b), float(dt), _dev(rhs, 8),
+                             _dev(y, 8), _stream(stream)))
+    return y
+
+
+def set_fallback_counter(counter):
+    """counter: CUDA int64 tensor of one element (caller-zeroed) or None to switch counting off."""
+    _check(lib().grx_debug_set_fallback_counter(C.c_void_p(counter.data_ptr()) if counter is not None else C.c_void_p(0)))
+
+
+def set_variant(name):
+    _check(lib().grx_set_variant(VARIANT[name] if isinstance(name, str) else int(name)))
+
+
+def selftest_math(x):
+    """Returns (1/x, 1/sqrt(x), sqrt(x)) computed with the kernels' division-free helpers."""
+    import torch
+    n = x.numel()
+    y = torch.empty(3 * n, dtype=torch.float64, device=x.device)
+    _check(lib().grx_selftest_math(_dev(x), _dev(y), n, _stream()))
+    return y[:n], y[n:2 * n], y[2 * n:]
+
+
+def dfma_peak_launch(iters, sink, stream=None):
+    """Launches the DFMA micro-benchmark once; returns the flop count of the launch."""
+    flops = C.c_double(0.0)
+    _check(lib().grx_dfma_peak_launch(int(iters), _dev(sink), C.byref(flops), _stream(stream)))
+    return flops.value
+
+
+def version():
+    return lib().grx_version()
+
+
+def weno_eps():
+    return lib().grx_weno_eps()
+
+
+def v2max():
+    return lib().grx_v2max()

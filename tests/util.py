@@ -74,3 +74,13 @@ def permute_problem(prob):
     dx = tuple(prob.dx[old_of_new[a]] for a in range(3))
     p2 = Problem(prob.name + "-perm", n, prob.nbox, prob.nghost, dx, prob.gamma, prim2, met2, K2)
     return p2, tr, old_of_new
+
+
+def cut_block(prob, lo, n, box=None):
+    """Sub-block of `n` interior cells starting at interior cell `lo`, with its ghost shell taken from the
+    surrounding data (so even a 1x1x1 block has non-trivial neighbours)."""
+    g = prob.nghost
+    sl = (slice(None) if box is None else slice(box, box + 1), slice(None),
+          slice(lo[2], lo[2] + n[2] + 2 * g), slice(lo[1], lo[1] + n[1] + 2 * g), slice(lo[0], lo[0] + n[0] + 2 * g))
+    arrs = [np.ascontiguousarray(a[sl]) for a in (prob.prim, prob.metric, prob.K)]
+    return Problem(f"{prob.name}-cut{tuple(n)}", tuple(n), arrs[0].shape[0], g, prob.dx, prob.gamma, *arrs)
