@@ -171,6 +171,9 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
         const bool xr = (TY <= 16) && lane >= TY && (lane - TY) < tye;
         const int xrow = xl ? lane : lane - TY;
         const bool ycol = lane < txe;
+        // a rim face is the first face of the next tile too: only the block's last faces are counted here
+        const bool count_x = (X0 + txe == p.n[0]), count_y = (Y0 + tye == p.n[1]);
+        unsigned dup = 0;
         for (int kk = 0; kk < nk; ++kk) {
             const long long cp = cbase + sz * (kk + 1);   // tile origin in plane k0+kk
             double yb_qp[8], yt_qm[8], xr_qm[8];
@@ -197,7 +200,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 double PL[8], Fh[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][xrow][txe];
-                face8<0>(prim, met, nc, cxr - 1, cxr, PL, xr_qm, gamma, Fh, nfb);
+                face8<0>(prim, met, nc, cxr - 1, cxr, PL, xr_qm, gamma, Fh, count_x ? nfb : dup);
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][xrow][txe] = Fh[q];
             }
@@ -211,7 +214,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 double PL[8], Fh[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][tye][lane];
-                face8<1>(prim, met, nc, cyt - sy, cyt, PL, yt_qm, gamma, Fh, nfb);
+                face8<1>(prim, met, nc, cyt - sy, cyt, PL, yt_qm, gamma, Fh, count_y ? nfb : dup);
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][tye][lane] = Fh[q];
             }
