@@ -231,7 +231,7 @@ struct Config { int ty, minb; };
 
 // GRX_TILE="<TY>x<MINB>" overrides the default tile (tuning knob; the compiled set is listed in dispatch()).
 Config pick_config() {
-    Config c = {7, 2};
+    Config c = {7, 1};
     if (const char* e = std::getenv("GRX_TILE")) {
         int ty = 0, mb = 0;
         if (std::sscanf(e, "%dx%d", &ty, &mb) == 2) { c.ty = ty; c.minb = mb; }
