@@ -68,8 +68,10 @@ int grx_valencia_rhs(const grx_grid* grid, const double* prim, const double* met
     p.gamma = gamma;
     p.nfallback = t_fallback_counter;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const cudaError_t e = (g_variant.load() == GRX_VARIANT_SIMPLE) ? grx::launch_rhs_simple(p, recon, st)
-                                                                   : grx::launch_rhs_fused(p, recon, st);
+    const int variant = g_variant.load();
+    const cudaError_t e = (variant == GRX_VARIANT_SIMPLE)  ? grx::launch_rhs_simple(p, recon, st)
+                          : (variant == GRX_VARIANT_SPLIT) ? grx::launch_rhs_split(p, recon, st)
+                                                           : grx::launch_rhs_fused(p, recon, st);
     if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs launch");
     return GRX_OK;
 }
@@ -149,7 +151,7 @@ int grx_debug_set_fallback_counter(unsigned long long* counter) {
 }
 
 int grx_set_variant(int variant) {
-    if (variant != GRX_VARIANT_FUSED && variant != GRX_VARIANT_SIMPLE) return fail(GRX_ERR_INVALID_ARG, "unknown variant");
+    if (variant != GRX_VARIANT_FUSED && variant != GRX_VARIANT_SIMPLE && variant != GRX_VARIANT_SPLIT) return fail(GRX_ERR_INVALID_ARG, "unknown variant");
     g_variant.store(variant);
     return GRX_OK;
 }

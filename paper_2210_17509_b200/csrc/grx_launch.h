@@ -12,6 +12,9 @@ cudaError_t launch_rhs_simple(const RhsParams& p, int recon, cudaStream_t st);
 // grx_fused.cu: the product kernel
 cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st);
 
+// grx_split.cu: two barrier-free kernels (z + sources, then x + y)
+cudaError_t launch_rhs_split(const RhsParams& p, int recon, cudaStream_t st);
+
 // grx_support.cu
 cudaError_t launch_prim2con(const double* prim, const double* met, long long nc, int nbox, double gamma, double* cons,
                             cudaStream_t st);

@@ -30,18 +30,17 @@ constexpr double V2MAX    = 1.0 - 1e-4;  // admissibility bound on v^2 (W_max = 
 enum { RECON_MINMOD = 0, RECON_MC = 1, RECON_WENO5 = 2 };
 
 // ---- reciprocal, reciprocal square root, square root without the IEEE slow paths ----------------------
-// MUFU.RCP64H / MUFU.RSQ64H give ~20+ good bits; one third-order step brings the relative error to
-// ~1e-17 (grx_selftest_math + tests/test_gpu_parity.py::test_selftest_math measure it).  Arguments are
-// positive, normal numbers everywhere these are used (determinants, lapse, rho h*, 1 - v^2 a^2, ...).
+// MUFU.RCP64H / MUFU.RSQ64H seeds are good to 2^-19.9 / 2^-20.1 (measured on B200 over 2^-30..2^30, see
+// profiles/r1_microbench.md); ONE third-order correction brings the relative error to 2.2e-16 / 2.6e-16,
+// i.e. the rounding level of the IEEE operation (grx_selftest_math + tests/test_gpu_parity.py measure it).
+// Arguments are positive, normal numbers everywhere these are used (determinants, lapse, rho h*, ...).
 GRX_HD double rcp(double x) {
 #if defined(__CUDA_ARCH__)
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double e = fma(-x, y, 1.0);
-    double e2 = fma(e, e, e);
-    y = fma(y, e2, y);
-    e = fma(-x, y, 1.0);          // one Newton step on top: keeps 0.5 ulp-level accuracy even if the seed
-    return fma(y, e, y);          // is only 2^-14 good
+    const double e = fma(-x, y, 1.0);
+    const double e2 = fma(e, e, e);
+    return fma(y, e2, y);                       // y (1 + e + e^2)
 #else
     return 1.0 / x;
 #endif
@@ -50,21 +49,23 @@ GRX_HD double rsqrt(double x) {
 #if defined(__CUDA_ARCH__)
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double t = x * y;
-    double h = fma(-t, y, 1.0);                 // 1 - x y^2
-    double p = fma(0.375, h, 0.5);
-    y = fma(y * h, p, y);                       // y (1 + h/2 + 3h^2/8)
-    t = x * y;
-    h = fma(-t, y, 1.0);
-    return fma(0.5 * y, h, y);                  // Newton step on top
+    const double t = x * y;
+    const double h = fma(-t, y, 1.0);           // 1 - x y^2
+    const double p = fma(0.375, h, 0.5);
+    return fma(y * h, p, y);                    // y (1 + h/2 + 3h^2/8)
 #else
     return 1.0 / sqrt(x);
 #endif
 }
-// sqrt of a non-negative number (0 -> 0)
+// sqrt of a non-negative number (0 -> 0): g = x y ~ sqrt(x), corrected to third order in h = 1 - g y
 GRX_HD double sqrt_nn(double x) {
 #if defined(__CUDA_ARCH__)
-    double s = x * rsqrt(x);
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double g = x * y;
+    const double h = fma(-g, y, 1.0);
+    const double p = fma(0.375, h, 0.5);
+    const double s = fma(g * h, p, g);
     return (x > 0.0) ? s : 0.0;
 #else
     return sqrt(x);
@@ -216,17 +217,19 @@ GRX_HD void side_state(const double Pin[8], const double* __restrict__ cen, long
     F[6] = fma(cBy, avd, -cBd * avy);
     F[7] = fma(cBz, avd, -cBd * avz);
     F[5 + D] = 0.0;
-    // fast-magnetosonic speeds (R8): a^2 = cs^2 + vA^2 - cs^2 vA^2 = (b^2 + Gamma p)/(rho h*)
+    // fast-magnetosonic speeds (R8).  With N = b^2 + Gamma p, M = rho h - Gamma p, rho h* = N + M:
+    //   a^2 = N/(rho h*), 1 - a^2 = M/(rho h*), 1 - v^2 a^2 = Dn/(rho h*) with Dn = rho h* - v^2 N, so
+    //   lambda^+- = alpha [v^d M +- sqrt(N (1 - v^2) (gamma^dd Dn - v^d v^d M))] / Dn - beta^d
+    // (the factors 1/(rho h*) cancel: one reciprocal, one square root, no cancellation in 1 - a^2).
     const double gp = gamma * p;
-    const double irhohs = rcp(rhohs);
-    const double a2 = (b2 + gp) * irhohs;
-    const double oma2 = (rhoh - gp) * irhohs;                // 1 - a^2
-    const double den = fma(-v2, a2, 1.0);                    // 1 - v^2 a^2
-    const double iden = rcp(den);
-    const double disc = a2 * iW2 * fma(m.gdd, den, -vd * vd * oma2);
+    const double N = b2 + gp;
+    const double M = rhoh - gp;
+    const double Dn = fma(-v2, N, rhohs);
+    const double iDn = rcp(Dn);
+    const double disc = (N * iW2) * fma(m.gdd, Dn, -(vd * vd) * M);
     const double root = sqrt_nn(fmax(disc, 0.0));
-    const double c0 = vd * oma2;
-    const double ai = alp * iden;
+    const double c0 = vd * M;
+    const double ai = alp * iDn;
     const double bd = m.beta[D];
     lam_p = fma(ai, c0 + root, -bd);
     lam_m = fma(ai, c0 - root, -bd);
@@ -236,14 +239,15 @@ GRX_HD void side_state(const double Pin[8], const double* __restrict__ cen, long
 // m holds the averaged alp, beta, g on entry; cenL/cenR point at field 0 of the two donor cells (field stride nc).
 template <int D>
 GRX_HD void face_flux(FaceGeom& m, const double PL[8], const double PR[8], const double* __restrict__ cenL,
-                      const double* __restrict__ cenR, long long nc, double gamma, double Fh[8], unsigned& nfallback) {
+                      const double* __restrict__ cenR, long long nc, double gamma, double Fh[8], unsigned& nfallback,
+                      double scale = 1.0) {
     face_geom_complete<D>(m);
     double UL[8], FL[8], UR[8], FR[8], lmL, lpL, lmR, lpR;
     side_state<D>(PL, cenL, nc, m, gamma, UL, FL, lmL, lpL, nfallback);
     side_state<D>(PR, cenR, nc, m, gamma, UR, FR, lmR, lpR, nfallback);
     const double lm = fmin(0.0, fmin(lmL, lmR));
     const double lp = fmax(0.0, fmax(lpL, lpR));
-    const double idl = rcp(lp - lm);
+    const double idl = rcp(lp - lm) * scale;      // `scale` (1/dx_d) rides on the three HLLE coefficients
     const double cL = lp * idl, cR = -lm * idl, cU = lp * lm * idl;
 #pragma unroll
     for (int c = 0; c < 8; ++c) Fh[c] = fma(cL, FL[c], fma(cR, FR[c], cU * (UR[c] - UL[c])));
@@ -324,6 +328,81 @@ GRX_HD void sources_point(const double P[8], const double met[10], const double 
     const double Sda = fma(Sux, dm[0][0], fma(Suy, dm[1][0], Suz * dm[2][0]));
     Stau = sg * fma(alp, KS, -Sda);
 }
+
+// ---- a9 in pieces (same formulas as sources_point, arranged so that only one direction's ten metric
+// derivatives are live at a time): the cell's Eulerian-observer stress-energy first, then one call per direction.
+struct SrcState {
+    double alp, sg;        // lapse, sqrt(det gamma)
+    double E;              // rho h* W^2 - P* - (alpha b^0)^2
+    double Sl[3], Su[3];   // S_k, S^k
+    double S2[6];          // S^{kl}: xx xy xz yy yz zz
+};
+GRX_HD void sources_prepare(const double P[8], const double met[10], double gamma, SrcState& s) {
+    const double rho = P[0], vx = P[1], vy = P[2], vz = P[3], eps = P[4], Bx = P[5], By = P[6], Bz = P[7];
+    const double gxx = met[4], gxy = met[5], gxz = met[6], gyy = met[7], gyz = met[8], gzz = met[9];
+    const double cxx = fma(gyy, gzz, -gyz * gyz);
+    const double cxy = fma(gxz, gyz, -gxy * gzz);
+    const double cxz = fma(gxy, gyz, -gxz * gyy);
+    const double cyy = fma(gxx, gzz, -gxz * gxz);
+    const double cyz = fma(gxy, gxz, -gxx * gyz);
+    const double czz = fma(gxx, gyy, -gxy * gxy);
+    const double det = fma(gxx, cxx, fma(gxy, cxy, gxz * cxz));
+    const double rs = rsqrt(det);
+    const double idet = rs * rs;
+    const double vlx = fma(gxx, vx, fma(gxy, vy, gxz * vz));
+    const double vly = fma(gxy, vx, fma(gyy, vy, gyz * vz));
+    const double vlz = fma(gxz, vx, fma(gyz, vy, gzz * vz));
+    const double v2 = fma(vlx, vx, fma(vly, vy, vlz * vz));
+    const double iW2 = 1.0 - v2;
+    const double W = rsqrt(iW2), iW = W * iW2, W2 = W * W;
+    const double Blx = fma(gxx, Bx, fma(gxy, By, gxz * Bz));
+    const double Bly = fma(gxy, Bx, fma(gyy, By, gyz * Bz));
+    const double Blz = fma(gxz, Bx, fma(gyz, By, gzz * Bz));
+    const double B2 = fma(Blx, Bx, fma(Bly, By, Blz * Bz));
+    const double Bv = fma(Bx, vlx, fma(By, vly, Bz * vlz));
+    const double ab0 = W * Bv;
+    const double b2 = fma(B2, iW2, Bv * Bv);
+    const double rhoeps = rho * eps;
+    const double p = (gamma - 1.0) * rhoeps;
+    const double rhohs = fma(gamma, rhoeps, rho) + b2;
+    const double Ps = fma(0.5, b2, p);
+    const double X = rhohs * W2;
+    s.alp = met[0];
+    s.sg = det * rs;
+    s.E = fma(-ab0, ab0, X - Ps);
+    const double bux = fma(Bx, iW, ab0 * vx), buy = fma(By, iW, ab0 * vy), buz = fma(Bz, iW, ab0 * vz);
+    s.Sl[0] = fma(X, vlx, -ab0 * fma(Blx, iW, ab0 * vlx));
+    s.Sl[1] = fma(X, vly, -ab0 * fma(Bly, iW, ab0 * vly));
+    s.Sl[2] = fma(X, vlz, -ab0 * fma(Blz, iW, ab0 * vlz));
+    s.Su[0] = fma(X, vx, -ab0 * bux);
+    s.Su[1] = fma(X, vy, -ab0 * buy);
+    s.Su[2] = fma(X, vz, -ab0 * buz);
+    const double Pi = Ps * idet;   // P* gamma^{kl} = P*/det * cofactor
+    const double Xvx = X * vx, Xvy = X * vy, Xvz = X * vz;
+    s.S2[0] = fma(Xvx, vx, fma(Pi, cxx, -bux * bux));
+    s.S2[1] = fma(Xvx, vy, fma(Pi, cxy, -bux * buy));
+    s.S2[2] = fma(Xvx, vz, fma(Pi, cxz, -bux * buz));
+    s.S2[3] = fma(Xvy, vy, fma(Pi, cyy, -buy * buy));
+    s.S2[4] = fma(Xvy, vz, fma(Pi, cyz, -buy * buz));
+    s.S2[5] = fma(Xvz, vz, fma(Pi, czz, -buz * buz));
+}
+// Direction j: d[f] = 8 (m_{+1} - m_{-1}) - (m_{+2} - m_{-2}) of metric field f along j (unscaled, R12),
+// w = 1/(12 dx_j).  Returns S_{S_j} and adds -sqrt(gamma) S^j d_j alpha to Stau.
+GRX_HD double sources_dir(const SrcState& s, int j, const double d[10], double w, double& Stau) {
+    const double sdg = fma(s.S2[0], d[4], fma(s.S2[3], d[7], s.S2[5] * d[9])) * (0.5 * s.alp) +
+                       s.alp * fma(s.S2[1], d[5], fma(s.S2[2], d[6], s.S2[4] * d[8]));
+    const double sdb = fma(s.Sl[0], d[1], fma(s.Sl[1], d[2], s.Sl[2] * d[3]));
+    const double sw = s.sg * w;
+    Stau = fma(-sw * s.Su[j], d[0], Stau);
+    return sw * (sdg + fma(-s.E, d[0], sdb));
+}
+// The extrinsic-curvature term of S_tau: sqrt(gamma) alpha K_kl S^{kl}.
+GRX_HD double sources_K(const SrcState& s, const double K[6]) {
+    const double KS = fma(K[0], s.S2[0], fma(K[3], s.S2[3], K[5] * s.S2[5])) +
+                      2.0 * fma(K[1], s.S2[1], fma(K[2], s.S2[2], K[4] * s.S2[4]));
+    return s.sg * s.alp * KS;
+}
+GRX_HD double d4raw(double mm2, double mm1, double mp1, double mp2) { return fma(8.0, mp1 - mm1, -(mp2 - mm2)); }
 
 // ---- prim2con at one point with the full metric given (Eqs. 6-9) ----------------------------------------------
 GRX_HD void prim2con_point(const double P[8], const double met[10], double gamma, double U[8]) {
