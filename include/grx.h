@@ -48,7 +48,7 @@ enum { GRX_OK = 0, GRX_ERR_INVALID_ARG = 1, GRX_ERR_CUDA = 2, GRX_ERR_UNSUPPORTE
 
 /* Kernel variants (grx_set_variant).  GRX_VARIANT_FUSED is the product path; GRX_VARIANT_SIMPLE is a
  * one-thread-per-cell kernel that recomputes shared faces, kept as a cross-check of the fused one. */
-enum { GRX_VARIANT_FUSED = 0, GRX_VARIANT_SIMPLE = 1, GRX_VARIANT_SPLIT = 2 };
+enum { GRX_VARIANT_FUSED = 0, GRX_VARIANT_SIMPLE = 1, GRX_VARIANT_SPLIT = 2, GRX_VARIANT_STAGED = 3 };
 
 /* d/dt of the conserved variables on the interior cells of every box.
  *

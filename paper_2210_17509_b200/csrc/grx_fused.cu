@@ -25,7 +25,11 @@ constexpr int TX = 32;
 
 struct TileGeom {
     int ntx, nty, nzc, tz;   // tiles along x, y; z-chunks and their length
+    int pf;                  // software prefetch mode (tuning knob)
 };
+
+__device__ __forceinline__ void prefetch_l1(const double* a) { asm volatile("prefetch.global.L1 [%0];" ::"l"(a)); }
+__device__ __forceinline__ void prefetch_l2(const double* a) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a)); }
 
 // shared-memory exchange buffer: [8 fields][TY+1 rows][TX+1 columns]
 template <int TY>
@@ -94,6 +98,26 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
         for (int q = 0; q < 8; ++q) { qpz[q] = 0.0; acc[q] = 0.0; }
         for (int kk = -1; kk <= nk; ++kk, c += sz) {
+            if (tg.pf && active && kk < nk) {
+                // first touches of this column: metric plane k+2 (z derivative at the end of THIS step), K_ij of
+                // this plane, primitives of plane k+3 (z stencil at the top of the next step)
+                if (tg.pf & 1) {
+#pragma unroll
+                    for (int f = 0; f < 10; ++f) prefetch_l1(met + f * nc + c + 2 * sz);
+#pragma unroll
+                    for (int f = 0; f < 6; ++f) prefetch_l1(Kf + f * nc + c);
+                }
+                if (tg.pf & 2) {
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) prefetch_l1(prim + q * nc + c + 3 * sz);
+                }
+                if (tg.pf & 4) {
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) prefetch_l2(prim + q * nc + c + 5 * sz);
+#pragma unroll
+                    for (int f = 0; f < 10; ++f) prefetch_l2(met + f * nc + c + 4 * sz);
+                }
+            }
             if (active) {
                 // z: reconstruct this cell, close the face below it, finish the cell below
                 double qm[8], qp[8];
@@ -281,7 +305,9 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    const TileGeom tg = make_tiles(p, TY, sms * MINB);
+    TileGeom tg = make_tiles(p, TY, sms * MINB);
+    static const int pf = [] { const char* e = std::getenv("GRX_PREFETCH"); return e ? std::atoi(e) : 3; }();
+    tg.pf = pf;
     const dim3 grid((unsigned)(tg.ntx * tg.nty * tg.nzc), p.nbox);
     rhs_fused_kernel<RECON, TY, MINB><<<grid, (TY + 1) * 32, smem, st>>>(p, tg);
     return cudaGetLastError();
@@ -296,6 +322,9 @@ cudaError_t dispatch(const RhsParams& p, cudaStream_t st) {
     if (c.ty == 5 && c.minb == 2) return launch_one<RECON, 5, 2>(p, st);     // 2 x 192 threads, 168 regs
     if (c.ty == 15 && c.minb == 1) return launch_one<RECON, 15, 1>(p, st);   // 512 threads, 128 regs
     if (c.ty == 7 && c.minb == 1) return launch_one<RECON, 7, 1>(p, st);     // 256 threads, 255 regs
+    if (c.ty == 6 && c.minb == 1) return launch_one<RECON, 6, 1>(p, st);
+    if (c.ty == 3 && c.minb == 2) return launch_one<RECON, 3, 2>(p, st);
+    if (c.ty == 4 && c.minb == 2) return launch_one<RECON, 4, 2>(p, st);
     return cudaErrorInvalidConfiguration;
 }
 
