@@ -44,6 +44,8 @@ UNIT = "cell-updates/s"
 FLOPS_MODEL = {"weno5": (4753.0, 6209.0), "minmod": (2545.0, 1793.0), "mc": (2640.0, 1500.0)}
 # Nominal FP64 peak of a B200: 148 SMs x 64 FP64 lanes x 2 flop (FMA) x 1.965 GHz.
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+KERNEL_OF_VARIANT = {"fused": "rhs_fused_kernel", "staged": "rhs_staged_kernel", "simple": "rhs_simple_kernel",
+                     "split": "rhs_z_kernel + rhs_xy_kernel"}
 
 
 def algorithmic_flops_per_cell(n, recon):
@@ -264,6 +266,7 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     grx.lib()
+    grx.set_variant(args.variant)
     stream = torch.cuda.current_stream()
 
     prob = load_workload(args.workload, rank)
@@ -337,7 +340,7 @@ def run_ours(args):
     ach_gbs = by_cell * cells / t_launch / 1e9
     dfma = measure_dfma_peak(grx, torch, stream)
     roofline = {
-        "bound": "alu", "kernel": "rhs_fused_kernel", "achieved": ach_tflops, "peak": FP64_PEAK_NOMINAL_TFLOPS,
+        "bound": "alu", "kernel": KERNEL_OF_VARIANT[args.variant], "achieved": ach_tflops, "peak": FP64_PEAK_NOMINAL_TFLOPS,
         "unit": "TFLOP/s", "frac": ach_tflops / FP64_PEAK_NOMINAL_TFLOPS,
         "peak_source": "nominal FP64: 148 SM x 64 lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry)",
         "peak_dfma_measured": dfma, "frac_of_dfma_measured": ach_tflops / dfma if dfma > 0 else None,
@@ -366,12 +369,12 @@ def run_ours(args):
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"{prob.name} per GPU, {recon}+HLLE, Gamma-law EOS, perturbed conformally flat metric "
                                f"+ shift + K_ij, {g} ghosts; one grx_valencia_rhs call per step",
-                   "l2": "inputs 4.6 GB >> 126 MB L2, no flush", "tile": os.environ.get("GRX_TILE", "default"),
+                   "l2": "inputs 4.6 GB >> 126 MB L2, no flush", "tile": os.environ.get("GRX_TILE", "default"), "variant": args.variant,
                    "parallelism": f"blocks x{world}, no collective"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "matches_device_path": e2e_ok},
-        "gpu_launches": args.steps,
+        "gpu_launches": args.steps * (2 if args.variant == "split" else 1),
         "roofline": roofline,
         "cpu_baseline": cpu_baseline,
     }
@@ -388,6 +391,7 @@ def run_sweep(args):
     from paper_2210_17509_b200 import build, grx
     build.build()
     grx.lib()
+    grx.set_variant(args.variant)
     stream = torch.cuda.current_stream()
     for name in ("c5-32", "c5-64", "c5-128", "c5-256", "c4", "c3", "c2", "c1"):
         prob = load_workload(name, 0)
@@ -415,6 +419,8 @@ def main():
     ap.add_argument("--workload", default="c5-256")
     ap.add_argument("--recon", default="weno5", choices=["weno5", "minmod", "mc"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="wall-clock budget of the oracle sample")
+    ap.add_argument("--variant", default="fused", choices=["fused", "staged", "split", "simple"],
+                    help="kernel variant (fused = product path)")
     ap.add_argument("--sweep", action="store_true", help="time every config instead of the contract line")
     args = ap.parse_args()
     if args.steps < 1:

@@ -46,9 +46,12 @@ typedef struct {
 enum { GRX_RECON_MINMOD = 0, GRX_RECON_MC = 1, GRX_RECON_WENO5 = 2 };
 enum { GRX_OK = 0, GRX_ERR_INVALID_ARG = 1, GRX_ERR_CUDA = 2, GRX_ERR_UNSUPPORTED = 3 };
 
-/* Kernel variants (grx_set_variant).  GRX_VARIANT_FUSED is the product path; GRX_VARIANT_SIMPLE is a
- * one-thread-per-cell kernel that recomputes shared faces, kept as a cross-check of the fused one. */
-enum { GRX_VARIANT_FUSED = 0, GRX_VARIANT_SIMPLE = 1, GRX_VARIANT_SPLIT = 2, GRX_VARIANT_STAGED = 3 };
+/* Kernel variants (grx_set_variant).  GRX_VARIANT_FUSED is the product path.  The others compute the same
+ * function along a different traversal and are kept as cross-checks and as measured design alternatives
+ * (profiles/r1_variants.md): SIMPLE = one thread per cell, every thread evaluates its own six faces;
+ * SPLIT = two barrier-free kernels (z + sources, then x + y); STAGED = fused with the current plane staged in
+ * shared memory by cp.async; WS = fused plus a helper warp group for the source terms. */
+enum { GRX_VARIANT_FUSED = 0, GRX_VARIANT_SIMPLE = 1, GRX_VARIANT_SPLIT = 2, GRX_VARIANT_STAGED = 3, GRX_VARIANT_WS = 4 };
 
 /* d/dt of the conserved variables on the interior cells of every box.
  *

@@ -72,6 +72,7 @@ int grx_valencia_rhs(const grx_grid* grid, const double* prim, const double* met
     const cudaError_t e = (variant == GRX_VARIANT_SIMPLE)  ? grx::launch_rhs_simple(p, recon, st)
                           : (variant == GRX_VARIANT_SPLIT) ? grx::launch_rhs_split(p, recon, st)
                           : (variant == GRX_VARIANT_STAGED) ? grx::launch_rhs_staged(p, recon, st)
+                          : (variant == GRX_VARIANT_WS) ? grx::launch_rhs_ws(p, recon, st)
                                                            : grx::launch_rhs_fused(p, recon, st);
     if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs launch");
     return GRX_OK;
@@ -152,7 +153,7 @@ int grx_debug_set_fallback_counter(unsigned long long* counter) {
 }
 
 int grx_set_variant(int variant) {
-    if (variant != GRX_VARIANT_FUSED && variant != GRX_VARIANT_SIMPLE && variant != GRX_VARIANT_SPLIT && variant != GRX_VARIANT_STAGED) return fail(GRX_ERR_INVALID_ARG, "unknown variant");
+    if (variant != GRX_VARIANT_FUSED && variant != GRX_VARIANT_SIMPLE && variant != GRX_VARIANT_SPLIT && variant != GRX_VARIANT_STAGED && variant != GRX_VARIANT_WS) return fail(GRX_ERR_INVALID_ARG, "unknown variant");
     g_variant.store(variant);
     return GRX_OK;
 }

@@ -18,6 +18,9 @@ cudaError_t launch_rhs_split(const RhsParams& p, int recon, cudaStream_t st);
 // grx_staged.cu: fused kernel with the current plane staged in shared memory by cp.async
 cudaError_t launch_rhs_staged(const RhsParams& p, int recon, cudaStream_t st);
 
+// grx_ws.cu: fused kernel plus a helper warp group for the sources (setmaxnreg)
+cudaError_t launch_rhs_ws(const RhsParams& p, int recon, cudaStream_t st);
+
 // grx_support.cu
 cudaError_t launch_prim2con(const double* prim, const double* met, long long nc, int nbox, double gamma, double* cons,
                             cudaStream_t st);

@@ -1,25 +1,24 @@
-// grx_fused.cu -- the product kernel: reconstruct + HLLE + flux divergence in all three directions and the
-// geometric sources in ONE pass over the block (steps 2-4), every face flux computed
-// exactly once.
+// grx_ws.cu -- warp-specialised variant of the fused right-hand side (experimental, GRX_VARIANT_WS).
 //
-// Decomposition:
-//   * A CTA owns an in-plane tile of TX x TY cells (TX = 32 = one warp along x, TY warps along y) and
-//     MARCHES along z through a chunk of the block, one plane per step.
-//   * z-direction: each thread reconstructs its own cell along z and keeps q^+ of the previous plane in
-//     registers, so the face k-1/2 is evaluated once, by the thread that owns the column; the finished
-//     right-hand side of cell k-1 is stored at step k.
-//   * x- and y-direction: every thread reconstructs its own cell, publishes q^+ in shared memory, evaluates
-//     the face on its low side (from its neighbour's q^+ and its own q^-), publishes the flux, and takes the
-//     flux of its high face from its neighbour.  The faces and one-sided reconstructions on the rim of the
-//     tile belong to one extra "rim warp" per CTA, whose lanes run along the tile edges.
-//   * Sources: metric derivatives and the 3+1 source terms per cell, added to the same accumulators.
-// Global loads go through L1/L2 (__ldg); lanes run along x, so every load is a contiguous 256 B row segment.
+// Same tile/march/rim structure as grx_fused.cu, plus ONE EXTRA WARP GROUP (4 warps) per CTA that evaluates the
+// geometric sources (a8 + a9: 144 loads and ~290 FP64 operations per cell, the most load-heavy part of a step)
+// and hands S_x, S_y, S_z, S_tau to the flux warps through shared memory.  The flux warps take 176 registers,
+// the helper group 152 (setmaxnreg; 2 x 176 + 152 = 504 = 3 x 168, the launch allocation), so an SM holds 3 warps per scheduler instead of 2 and the
+// helpers' load phases overlap the flux warps' FP64 phases.  Named barriers: 1 = the 8 flux warps;
+// 2,3 = "sources of buffer b published"; 4,5 = "buffer b consumed".
 #include <cstdio>
 #include <cstdlib>
 
 #include "grx_launch.h"
 
 namespace grx {
+
+namespace {
+
+constexpr int WS_MAIN = 256, WS_ALL = 384;
+__device__ __forceinline__ void bar_main() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+__device__ __forceinline__ void bar_named_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_named_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
 constexpr int TX = 32;
 
@@ -64,12 +63,14 @@ __device__ __forceinline__ void face8(const double* __restrict__ prim, const dou
     face_flux<D>(m, PL, PR, prim + iL, prim + iR, nc, gamma, Fh, nfb);
 }
 
-template <int RECON, int TY, int MINB>
-__global__ void __launch_bounds__((TY + 1) * 32, MINB)
-rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
+template <int RECON, int TY>
+__global__ void __launch_bounds__((TY + 1) * 32 + 128, 1)
+rhs_ws_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
     extern __shared__ double smem_raw[];
     Exch<TY>& Qb = *reinterpret_cast<Exch<TY>*>(smem_raw);
     Exch<TY>& Fb = *reinterpret_cast<Exch<TY>*>(smem_raw + sizeof(Exch<TY>) / sizeof(double));
+    // sources hand-off: [buffer][S_x, S_y, S_z, S_tau][row][column]
+    double (*Ssrc)[4][TY][TX] = reinterpret_cast<double (*)[4][TY][TX]>(smem_raw + 2 * sizeof(Exch<TY>) / sizeof(double));
 
     int t = blockIdx.x;
     const int tix = t % tg.ntx; t /= tg.ntx;
@@ -80,6 +81,35 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
     const int txe = min(TX, p.n[0] - X0), tye = min(TY, p.n[1] - Y0);
     const int nk = min(tg.tz, p.n[2] - k0);       // planes owned by this CTA
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (warp > TY) {
+        // ------------------------------------------------ helper warp group: the geometric sources of the tile
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 152;");
+        const int h = warp - (TY + 1);
+        const int nc32 = (int)p.nc, sy32 = (int)p.stride[1], sz32 = (int)p.stride[2];
+        const long long c00 = (long long)blockIdx.y * p.nc;
+        const long long cell = (X0 + p.g + lane) + (long long)sy32 * (Y0 + p.g) + (long long)sz32 * (k0 + p.g);
+        const double* __restrict__ pc = p.prim + 8 * c00 + cell;
+        const double* __restrict__ mc = p.met + 10 * c00 + cell;
+        const double* __restrict__ kc = p.K + 6 * c00 + cell;
+        for (int kk = 0; kk < nk; ++kk, pc += sz32, mc += sz32, kc += sz32) {
+            const int b = kk & 1;
+            if (kk >= 2) bar_named_sync(4 + b, WS_ALL);          // the consumers are done with this buffer
+            for (int r = h; r < tye; r += 4) {
+                if (lane < txe) {
+                    double a[8];
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) a[q] = 0.0;
+                    sources_add(p, pc + r * sy32, mc + r * sy32, kc + r * sy32, nc32, sy32, sz32, a);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) Ssrc[b][q][r][lane] = a[1 + q];
+                }
+            }
+            __threadfence_block();
+            bar_named_arrive(2 + b, WS_ALL);                     // sources of plane k0+kk are in shared memory
+        }
+        return;
+    }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 176;");
 
     const double* __restrict__ prim = p.prim + (long long)box * 8 * p.nc;
     const double* __restrict__ met = p.met + (long long)box * 10 * p.nc;
@@ -149,7 +179,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Qb.v[q][warp][lane + 1] = qp[q];
             }
-            __syncthreads();
+            bar_main();
             if (active) {
                 double PL[8], Fh[8];
 #pragma unroll
@@ -158,7 +188,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][warp][lane] = Fh[q];
             }
-            __syncthreads();
+            bar_main();
             // y
             if (active) {
 #pragma unroll
@@ -168,7 +198,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Qb.v[q][warp + 1][lane] = qp[q];
             }
-            __syncthreads();
+            bar_main();
             if (active) {
                 double PL[8], Fh[8];
 #pragma unroll
@@ -177,13 +207,19 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][warp][lane] = Fh[q];
             }
-            __syncthreads();
+            bar_main();
             if (active) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) acc[q] = fma(Fb.v[q][warp][lane] - Fb.v[q][warp + 1][lane], p.idx[1], acc[q]);
-                double s1, s2, s3, s4;
-                sources_from_global(p, prim, met, Kf, c, s1, s2, s3, s4);
-                acc[1] += s1; acc[2] += s2; acc[3] += s3; acc[4] += s4;
+            }
+            {
+                const int b = kk & 1;
+                bar_named_sync(2 + b, WS_ALL);                    // the helper group has published this plane's sources
+                if (active) {
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) acc[1 + q] += Ssrc[b][q][warp][lane];
+                }
+                bar_named_arrive(4 + b, WS_ALL);
             }
         }
     } else {
@@ -219,7 +255,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) xr_qm[q] = qm[q];
             }
-            __syncthreads();
+            bar_main();
             if (xr) {
                 double PL[8], Fh[8];
 #pragma unroll
@@ -228,12 +264,12 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][xrow][txe] = Fh[q];
             }
-            __syncthreads();
+            bar_main();
             if (ycol) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Qb.v[q][0][lane] = yb_qp[q];
             }
-            __syncthreads();
+            bar_main();
             if (ycol) {
                 double PL[8], Fh[8];
 #pragma unroll
@@ -242,30 +278,16 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][tye][lane] = Fh[q];
             }
-            __syncthreads();
+            bar_main();
+            bar_named_sync(2 + (kk & 1), WS_ALL);                 // keep the hand-off barrier counts uniform
+            bar_named_arrive(4 + (kk & 1), WS_ALL);
         }
     }
     if (p.nfallback && nfb) atomicAdd(p.nfallback, (unsigned long long)nfb);
 }
 
-// ---- host side ------------------------------------------------------------------------------------------------
-namespace {
 
-struct Config { int ty, minb; };
-
-// GRX_TILE="<TY>x<MINB>" overrides the default tile (tuning knob; the compiled set is listed in dispatch()).
-Config pick_config() {
-    Config c = {7, 1};
-    if (const char* e = std::getenv("GRX_TILE")) {
-        int ty = 0, mb = 0;
-        if (std::sscanf(e, "%dx%d", &ty, &mb) == 2) { c.ty = ty; c.minb = mb; }
-    }
-    return c;
-}
-
-// z-chunking: enough CTAs to fill the machine a few times over, chunks long enough to amortise the two
-// one-sided plane steps at their ends.
-TileGeom make_tiles(const RhsParams& p, int ty, int slots) {
+TileGeom make_tiles_ws(const RhsParams& p, int ty, int slots) {
     TileGeom tg;
     tg.ntx = (p.n[0] + TX - 1) / TX;
     tg.nty = (p.n[1] + ty - 1) / ty;
@@ -275,8 +297,7 @@ TileGeom make_tiles(const RhsParams& p, int ty, int slots) {
     const int maxc = (p.n[2] + 7) / 8;
     for (int nzc = 1; nzc <= maxc; ++nzc) {
         const int tz = (p.n[2] + nzc - 1) / nzc;
-        const int real = (p.n[2] + tz - 1) / tz;
-        if (real != nzc) continue;
+        if ((p.n[2] + tz - 1) / tz != nzc) continue;
         const double waves = (double)(inplane * nzc) / slots;
         const double fill = waves / (double)(long long)(waves + 0.999999);
         const double eff = fill * tz / (tz + 0.45);
@@ -284,11 +305,13 @@ TileGeom make_tiles(const RhsParams& p, int ty, int slots) {
     }
     tg.tz = (p.n[2] + best - 1) / best;
     tg.nzc = (p.n[2] + tg.tz - 1) / tg.tz;
+    tg.pf = 3;
     return tg;
 }
 
-template <int RECON, int TY, int MINB>
-cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
+template <int RECON>
+cudaError_t launch_ws_t(const RhsParams& p, cudaStream_t st) {
+    constexpr int TY = 7;
     static int sms = 0;
     if (sms == 0) {
         int dev = 0;
@@ -297,41 +320,25 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
         e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return e;
     }
-    const size_t smem = 2 * sizeof(Exch<TY>);
+    const size_t smem = 2 * sizeof(Exch<TY>) + 2 * 4 * TY * TX * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(rhs_fused_kernel<RECON, TY, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(rhs_ws_kernel<RECON, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    TileGeom tg = make_tiles(p, TY, sms * MINB);
-    static const int pf = [] { const char* e = std::getenv("GRX_PREFETCH"); return e ? std::atoi(e) : 3; }();
-    tg.pf = pf;
+    const TileGeom tg = make_tiles_ws(p, TY, sms);
     const dim3 grid((unsigned)(tg.ntx * tg.nty * tg.nzc), p.nbox);
-    rhs_fused_kernel<RECON, TY, MINB><<<grid, (TY + 1) * 32, smem, st>>>(p, tg);
+    rhs_ws_kernel<RECON, TY><<<grid, (TY + 1) * 32 + 128, smem, st>>>(p, tg);
     return cudaGetLastError();
-}
-
-template <int RECON>
-cudaError_t dispatch(const RhsParams& p, cudaStream_t st) {
-    const Config c = pick_config();
-    // compiled tiles: TY regular warps + 1 rim warp per CTA, MINB CTAs per SM (-> register budget)
-    if (c.ty == 7 && c.minb == 2) return launch_one<RECON, 7, 2>(p, st);     // 2 x 256 threads, 128 regs
-    if (c.ty == 11 && c.minb == 1) return launch_one<RECON, 11, 1>(p, st);   // 384 threads, 168 regs
-    if (c.ty == 5 && c.minb == 2) return launch_one<RECON, 5, 2>(p, st);     // 2 x 192 threads, 168 regs
-    if (c.ty == 15 && c.minb == 1) return launch_one<RECON, 15, 1>(p, st);   // 512 threads, 128 regs
-    if (c.ty == 7 && c.minb == 1) return launch_one<RECON, 7, 1>(p, st);     // 256 threads, 255 regs
-    if (c.ty == 6 && c.minb == 1) return launch_one<RECON, 6, 1>(p, st);     // 224 threads, 255 regs
-    return cudaErrorInvalidConfiguration;
 }
 
 }  // namespace
 
-cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st) {
-    if (recon == RECON_WENO5) return dispatch<RECON_WENO5>(p, st);
-    if (recon == RECON_MC) return dispatch<RECON_MC>(p, st);
-    return dispatch<RECON_MINMOD>(p, st);
+cudaError_t launch_rhs_ws(const RhsParams& p, int recon, cudaStream_t st) {
+    if (recon == RECON_WENO5) return launch_ws_t<RECON_WENO5>(p, st);
+    if (recon == RECON_MC) return launch_ws_t<RECON_MC>(p, st);
+    return launch_ws_t<RECON_MINMOD>(p, st);
 }
 
 }  // namespace grx

@@ -63,7 +63,7 @@ def check(prob, recon, got, ref, tol=TOL):
 SMALL = ["c1", "gen", "c2:small", "c3:small", "c4:small", "c5-32:small"]
 
 
-@pytest.mark.parametrize("variant", ["fused", "simple"])
+@pytest.mark.parametrize("variant", ["fused", "simple", "split", "staged", "ws"])
 @pytest.mark.parametrize("name", SMALL)
 def test_parity_small(grx, oracle, name, variant):
     prob = inputs.by_name(name)
@@ -74,7 +74,38 @@ def test_parity_small(grx, oracle, name, variant):
         assert nfb == nfb_ref, f"{name}/{recon}: fallback count {nfb} vs oracle {nfb_ref} (R5)"
 
 
-@pytest.mark.parametrize("tile", ["7x2", "11x1", "5x2", "15x1", "7x1"])
+@pytest.mark.parametrize("variant", ["split", "staged", "ws"])
+@pytest.mark.parametrize("n", [(1, 5, 2), (33, 1, 3), (2, 2, 70), (65, 8, 9), (31, 61, 17)])
+def test_parity_variants_ragged(grx, oracle, variant, n):
+    """The split (two barrier-free kernels), staged (cp.async plane in shared memory) and ws (helper warp group
+    for the sources) variants on ragged
+    and thin blocks with an off-diagonal metric: sizes off the 30/32-cell tiles, single rows, long columns."""
+    base = inputs.general_metric_box(n=(66, 62, 71), seed=3, nbox=2)
+    prob = cut_block(base, (1, 1, 1), n)
+    for recon in ("minmod", "weno5"):
+        ref, nfb_ref = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, prob.nghost, recon, prob.gamma)
+        got, nfb = gpu_rhs(grx, prob, recon, variant, count=True)
+        check(prob, recon, got, ref)
+        assert nfb == nfb_ref
+
+
+@pytest.mark.parametrize("variant", ["split", "staged", "ws"])
+def test_parity_variants_two_ghosts_and_rotor(grx, oracle, variant):
+    """minmod/MC with the minimal 2 ghosts (the staged halo must not read outside the array) and the rotor's
+    inadmissible WENO5 face states (R5) through the variants."""
+    prob = inputs.general_metric_box(n=(18, 10, 7), seed=21, g=2)
+    for recon in ("minmod", "mc"):
+        ref, _ = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, 2, recon, prob.gamma)
+        check(prob, recon, gpu_rhs(grx, prob, recon, variant), ref)
+    prob = inputs.rotor((96, 80, 1))
+    for recon in prob.recons:
+        ref, nfb_ref = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, prob.nghost, recon, prob.gamma)
+        got, nfb = gpu_rhs(grx, prob, recon, variant, count=True)
+        check(prob, recon, got, ref)
+        assert nfb == nfb_ref
+
+
+@pytest.mark.parametrize("tile", ["7x2", "11x1", "5x2", "15x1", "7x1", "6x1"])
 def test_parity_all_tiles(grx, oracle, tile, monkeypatch):
     """Every compiled tile shape of the fused kernel, on a ragged off-diagonal-metric batch and the rotor."""
     monkeypatch.setenv("GRX_TILE", tile)
@@ -188,9 +219,10 @@ def test_fused_equals_simple_variant(grx):
     prob = inputs.general_metric_box(n=(40, 17, 13), seed=5, nbox=3)
     for recon in ("minmod", "mc", "weno5"):
         a = gpu_rhs(grx, prob, recon, "fused")
-        b = gpu_rhs(grx, prob, recon, "simple")
         ii = prob.interior
-        assert relerr_per_component(a[ii], b[ii]).max() < 1e-13
+        for other in ("simple", "split", "staged", "ws"):
+            b = gpu_rhs(grx, prob, recon, other)
+            assert relerr_per_component(a[ii], b[ii]).max() < 1e-13, other
 
 
 def test_batch_equals_single_boxes_bitwise(grx):
