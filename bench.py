@@ -45,7 +45,7 @@ FLOPS_MODEL = {"weno5": (4753.0, 6209.0), "minmod": (2545.0, 1793.0), "mc": (264
 # Nominal FP64 peak of a B200: 148 SMs x 64 FP64 lanes x 2 flop (FMA) x 1.965 GHz.
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 KERNEL_OF_VARIANT = {"fused": "rhs_fused_kernel", "staged": "rhs_staged_kernel", "simple": "rhs_simple_kernel",
-                     "split": "rhs_z_kernel + rhs_xy_kernel"}
+                     "split": "rhs_z_kernel + rhs_xy_kernel", "ws": "rhs_ws_kernel"}
 
 
 def algorithmic_flops_per_cell(n, recon):
@@ -419,7 +419,7 @@ def main():
     ap.add_argument("--workload", default="c5-256")
     ap.add_argument("--recon", default="weno5", choices=["weno5", "minmod", "mc"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="wall-clock budget of the oracle sample")
-    ap.add_argument("--variant", default="fused", choices=["fused", "staged", "split", "simple"],
+    ap.add_argument("--variant", default="fused", choices=["fused", "staged", "split", "ws", "simple"],
                     help="kernel variant (fused = product path)")
     ap.add_argument("--sweep", action="store_true", help="time every config instead of the contract line")
     args = ap.parse_args()

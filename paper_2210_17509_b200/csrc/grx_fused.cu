@@ -94,9 +94,13 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
         // ------------------------------------------------ regular warp: one cell column per thread
         const bool active = (lane < txe) && (warp < tye);
         long long c = cbase + lane + sy * warp;
-        double qpz[8], acc[8];
+        // q^+ of the previous plane waits in a thread-private shared-memory slot between two z faces (it is
+        // needed once per step; parking it frees 16 registers during the x, y and source phases)
+        volatile double* zpark = smem_raw + 2 * sizeof(Exch<TY>) / sizeof(double) + threadIdx.x;
+        constexpr int ZS = (TY + 1) * 32;
+        double acc[8];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) { qpz[q] = 0.0; acc[q] = 0.0; }
+        for (int q = 0; q < 8; ++q) acc[q] = 0.0;
         for (int kk = -1; kk <= nk; ++kk, c += sz) {
             if (tg.pf && active && kk < nk) {
                 // first touches of this column: metric plane k+2 (z derivative at the end of THIS step), K_ij of
@@ -126,6 +130,9 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                     double Fh[8];
                     // the first face of an inner chunk is also the last face of the chunk below: count once
                     unsigned dup = 0;
+                    double qpz[8];
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) qpz[q] = zpark[q * ZS];
                     face8<2>(prim, met, nc, c - sz, c, qpz, qm, gamma, Fh, (kk == 0 && k0 > 0) ? dup : nfb);
                     // F/dz is rounded once and used with both signs, so a uniform state cancels exactly
 #pragma unroll
@@ -138,7 +145,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                     for (int q = 0; q < 8; ++q) acc[q] = Fh[q];
                 }
 #pragma unroll
-                for (int q = 0; q < 8; ++q) qpz[q] = qp[q];
+                for (int q = 0; q < 8; ++q) zpark[q * ZS] = qp[q];
             }
             if (kk < 0 || kk >= nk) continue;   // uniform over the CTA
             // x
@@ -255,7 +262,7 @@ struct Config { int ty, minb; };
 
 // GRX_TILE="<TY>x<MINB>" overrides the default tile (tuning knob; the compiled set is listed in dispatch()).
 Config pick_config() {
-    Config c = {7, 1};
+    Config c = {11, 1};
     if (const char* e = std::getenv("GRX_TILE")) {
         int ty = 0, mb = 0;
         if (std::sscanf(e, "%dx%d", &ty, &mb) == 2) { c.ty = ty; c.minb = mb; }
@@ -297,7 +304,7 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
         e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return e;
     }
-    const size_t smem = 2 * sizeof(Exch<TY>);
+    const size_t smem = 2 * sizeof(Exch<TY>) + 8 * (TY + 1) * 32 * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(rhs_fused_kernel<RECON, TY, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
