@@ -64,6 +64,12 @@ __device__ __forceinline__ void face8(const double* __restrict__ prim, const dou
     face_flux<D>(m, PL, PR, prim + iL, prim + iR, nc, gamma, Fh, nfb);
 }
 
+// The running sum of the cell being finished also waits in thread-private shared memory between the points
+// where it is updated (4 per step): with the z carry that keeps 32 registers free during the face evaluations.
+#define GRX_ACC_LOAD _Pragma("unroll") for (int q_ = 0; q_ < 8; ++q_) acc[q_] = apark[q_ * ((TY + 1) * 32)];
+#define GRX_ACC_STORE _Pragma("unroll") for (int q_ = 0; q_ < 8; ++q_) apark[q_ * ((TY + 1) * 32)] = acc[q_];
+constexpr int PARK_SLOTS = 16;   // doubles per thread: z carry q^+[8], running sum[8]
+
 template <int RECON, int TY, int MINB>
 __global__ void __launch_bounds__((TY + 1) * 32, MINB)
 rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
@@ -89,6 +95,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
     const double gamma = p.gamma;
     const long long cbase = (X0 + p.g) + sy * (Y0 + p.g) + sz * (k0 - 1 + p.g);   // tile origin, plane k0-1
     unsigned nfb = 0;
+    volatile double* apark = smem_raw + 2 * sizeof(Exch<TY>) / sizeof(double) + 8 * (TY + 1) * 32 + threadIdx.x;
 
     if (warp < TY) {
         // ------------------------------------------------ regular warp: one cell column per thread
@@ -138,11 +145,13 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                     for (int q = 0; q < 8; ++q) Fh[q] = __dmul_rn(Fh[q], p.idx[2]);
                     if (kk >= 1) {
+                        GRX_ACC_LOAD
 #pragma unroll
                         for (int q = 0; q < 8; ++q) out[q * nc + c - sz] = __dsub_rn(acc[q], Fh[q]);
                     }
 #pragma unroll
                     for (int q = 0; q < 8; ++q) acc[q] = Fh[q];
+                    GRX_ACC_STORE
                 }
 #pragma unroll
                 for (int q = 0; q < 8; ++q) zpark[q * ZS] = qp[q];
@@ -168,8 +177,10 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
             __syncthreads();
             // y
             if (active) {
+                GRX_ACC_LOAD
 #pragma unroll
                 for (int q = 0; q < 8; ++q) acc[q] = fma(Fb.v[q][warp][lane] - Fb.v[q][warp][lane + 1], p.idx[0], acc[q]);
+                GRX_ACC_STORE
                 double qp[8];
                 recon8<RECON>(prim, nc, c, sy, qm, qp);
 #pragma unroll
@@ -186,11 +197,13 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
             }
             __syncthreads();
             if (active) {
+                GRX_ACC_LOAD
 #pragma unroll
                 for (int q = 0; q < 8; ++q) acc[q] = fma(Fb.v[q][warp][lane] - Fb.v[q][warp + 1][lane], p.idx[1], acc[q]);
                 double s1, s2, s3, s4;
                 sources_from_global(p, prim, met, Kf, c, s1, s2, s3, s4);
                 acc[1] += s1; acc[2] += s2; acc[3] += s3; acc[4] += s4;
+                GRX_ACC_STORE
             }
         }
     } else {
@@ -261,8 +274,11 @@ namespace {
 struct Config { int ty, minb; };
 
 // GRX_TILE="<TY>x<MINB>" overrides the default tile (tuning knob; the compiled set is listed in dispatch()).
-Config pick_config() {
+// Default: 11 rows (12 warps per SM at 168 registers, fastest on every 3-D block of the sweep); blocks that are
+// thin along z have too few plane steps per CTA to amortise the taller tile and take the 7-row one.
+Config pick_config(const RhsParams& p) {
     Config c = {11, 1};
+    if (p.n[2] < 8) c.ty = 7;
     if (const char* e = std::getenv("GRX_TILE")) {
         int ty = 0, mb = 0;
         if (std::sscanf(e, "%dx%d", &ty, &mb) == 2) { c.ty = ty; c.minb = mb; }
@@ -304,7 +320,7 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
         e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return e;
     }
-    const size_t smem = 2 * sizeof(Exch<TY>) + 8 * (TY + 1) * 32 * sizeof(double);
+    const size_t smem = 2 * sizeof(Exch<TY>) + PARK_SLOTS * (TY + 1) * 32 * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(rhs_fused_kernel<RECON, TY, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -322,7 +338,7 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
 
 template <int RECON>
 cudaError_t dispatch(const RhsParams& p, cudaStream_t st) {
-    const Config c = pick_config();
+    const Config c = pick_config(p);
     // compiled tiles: TY regular warps + 1 rim warp per CTA, MINB CTAs per SM (-> register budget)
     if (c.ty == 7 && c.minb == 2) return launch_one<RECON, 7, 2>(p, st);     // 2 x 256 threads, 128 regs
     if (c.ty == 11 && c.minb == 1) return launch_one<RECON, 11, 1>(p, st);   // 384 threads, 168 regs
