@@ -79,12 +79,15 @@ int grx_valencia_rhs(const grx_grid* grid, const double* prim, const double* met
                      const double dx[3], int nghost, int recon, double gamma, double* out, void* cuda_stream);
 
 /* Same computation for HOST arrays (end-to-end entry point): copies prim, metric and K to the device
- * workspace, runs grx_valencia_rhs there and copies `out` back, all asynchronously on `cuda_stream`
- * (cudaMemcpyAsync; the host arrays should be page-locked for the copies to be asynchronous).  The host
- * arrays have the layout above.  The WHOLE out array is copied back (its ghost cells hold whatever the
- * workspace held).
+ * workspace, evaluates the right-hand side there and copies the result back.  Blocks with more than 32 planes
+ * along z are processed as a pipeline of 32-plane slabs: the upload of the next slab, the kernel of the current
+ * one and the download of the previous one overlap on three streams (two internal ones, created and destroyed
+ * per call, ordered after / before `cuda_stream` by events); the results are bitwise those of the device entry
+ * point.  Only the INTERIOR planes of `out_host` are written in that case (all of it, ghosts holding whatever
+ * the workspace held, for blocks of <= 32 planes or while a debug fallback counter is set).  The host arrays
+ * have the layout above and should be page-locked for the copies to be asynchronous.
  *   workspace        DEVICE pointer, at least grx_host_workspace_bytes(grid, nghost) bytes, owned by the caller.
- * Results are valid in out_host after the stream is synchronised. */
+ * Results are valid in out_host after `cuda_stream` is synchronised. */
 size_t grx_host_workspace_bytes(const grx_grid* grid, int nghost);
 int grx_valencia_rhs_host(const grx_grid* grid, const double* prim_host, const double* metric_host,
                           const double* K_host, const double dx[3], int nghost, int recon, double gamma,

@@ -3,6 +3,7 @@
 #include <atomic>
 #include <cstdio>
 #include <cstring>
+#include <vector>
 
 #include "../../include/grx.h"
 #include "grx_launch.h"
@@ -44,6 +45,16 @@ const char* make_geom(const grx_grid* grid, int nghost, grx::RhsParams& p) {
     return nullptr;
 }
 
+// Launches the selected kernel variant on a (sub-)block.
+cudaError_t launch_variant(const grx::RhsParams& p, int recon, cudaStream_t st) {
+    const int variant = g_variant.load();
+    return (variant == GRX_VARIANT_SIMPLE)   ? grx::launch_rhs_simple(p, recon, st)
+           : (variant == GRX_VARIANT_SPLIT)  ? grx::launch_rhs_split(p, recon, st)
+           : (variant == GRX_VARIANT_STAGED) ? grx::launch_rhs_staged(p, recon, st)
+           : (variant == GRX_VARIANT_WS)     ? grx::launch_rhs_ws(p, recon, st)
+                                             : grx::launch_rhs_fused(p, recon, st);
+}
+
 }  // namespace
 
 extern "C" {
@@ -68,12 +79,7 @@ int grx_valencia_rhs(const grx_grid* grid, const double* prim, const double* met
     p.gamma = gamma;
     p.nfallback = t_fallback_counter;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const int variant = g_variant.load();
-    const cudaError_t e = (variant == GRX_VARIANT_SIMPLE)  ? grx::launch_rhs_simple(p, recon, st)
-                          : (variant == GRX_VARIANT_SPLIT) ? grx::launch_rhs_split(p, recon, st)
-                          : (variant == GRX_VARIANT_STAGED) ? grx::launch_rhs_staged(p, recon, st)
-                          : (variant == GRX_VARIANT_WS) ? grx::launch_rhs_ws(p, recon, st)
-                                                           : grx::launch_rhs_fused(p, recon, st);
+    const cudaError_t e = launch_variant(p, recon, st);
     if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs launch");
     return GRX_OK;
 }
@@ -91,8 +97,17 @@ int grx_valencia_rhs_host(const grx_grid* grid, const double* prim_host, const d
     grx::RhsParams p;
     std::memset(&p, 0, sizeof(p));
     if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
-    if (!prim_host || !metric_host || !K_host || !out_host || !workspace)
+    if (!prim_host || !metric_host || !K_host || !out_host || !workspace || !dx)
         return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (recon != GRX_RECON_MINMOD && recon != GRX_RECON_MC && recon != GRX_RECON_WENO5)
+        return fail(GRX_ERR_INVALID_ARG, "unknown recon");
+    if (nghost < (recon == GRX_RECON_WENO5 ? 3 : 2))
+        return fail(GRX_ERR_INVALID_ARG, "nghost too small: WENO5 needs 3, minmod/MC need 2 (R29)");
+    if (!(gamma > 1.0)) return fail(GRX_ERR_INVALID_ARG, "gamma must be > 1");
+    for (int a = 0; a < 3; ++a) {
+        if (!(dx[a] > 0.0) || !(1.0 / dx[a] > 0.0)) return fail(GRX_ERR_INVALID_ARG, "dx must be > 0 and finite");
+        p.idx[a] = 1.0 / dx[a];
+    }
     const size_t cells = (size_t)p.nc * (size_t)p.nbox;
     if (workspace_bytes < 32 * cells * sizeof(double)) return fail(GRX_ERR_INVALID_ARG, "workspace too small");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -100,14 +115,91 @@ int grx_valencia_rhs_host(const grx_grid* grid, const double* prim_host, const d
     double* d_met = d_prim + 8 * cells;
     double* d_K = d_met + 10 * cells;
     double* d_out = d_K + 6 * cells;
-    cudaError_t e = cudaMemcpyAsync(d_prim, prim_host, 8 * cells * sizeof(double), cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_met, metric_host, 10 * cells * sizeof(double), cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_K, K_host, 6 * cells * sizeof(double), cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_host H2D");
-    const int rc = grx_valencia_rhs(grid, d_prim, d_met, d_K, dx, nghost, recon, gamma, d_out, cuda_stream);
-    if (rc != GRX_OK) return rc;
-    e = cudaMemcpyAsync(out_host, d_out, 8 * cells * sizeof(double), cudaMemcpyDeviceToHost, st);
-    if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_host D2H");
+    p.prim = d_prim; p.met = d_met; p.K = d_K; p.out = d_out;
+    p.gamma = gamma;
+    p.nfallback = t_fallback_counter;
+
+    // Slab pipeline along z: the upload of planes [j*CH, (j+1)*CH) runs on its own stream; slab i (interior
+    // planes [i*CH, (i+1)*CH)) is evaluated on the caller's stream as soon as the planes it reads (up to
+    // (i+1)*CH + 2g - 1) have arrived; its result goes back on a third stream.  H2D, kernels and D2H overlap;
+    // every cell sees the same arithmetic as in the single-launch path (bitwise identical results).
+    const int CH = 32;
+    const int Nz = p.N[2], nz = p.n[2], g = p.g;
+    const bool pipelined = (nz > CH) && (2 * g <= CH) && (t_fallback_counter == nullptr);
+    if (!pipelined) {
+        cudaError_t e = cudaMemcpyAsync(d_prim, prim_host, 8 * cells * sizeof(double), cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_met, metric_host, 10 * cells * sizeof(double), cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_K, K_host, 6 * cells * sizeof(double), cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_host H2D");
+        e = launch_variant(p, recon, st);
+        if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_host launch");
+        e = cudaMemcpyAsync(out_host, d_out, 8 * cells * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_host D2H");
+        return GRX_OK;
+    }
+    cudaStream_t s_up = nullptr, s_dn = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_dn = nullptr;
+    // a tail shorter than 8 planes joins the last full slab, so that every slab takes the same tile as the whole block
+    const int nchunk = (Nz + CH - 1) / CH, nslab = (nz % CH != 0 && nz % CH < 8) ? nz / CH : (nz + CH - 1) / CH;
+    std::vector<cudaEvent_t> ev_up(nchunk, nullptr), ev_done(nslab, nullptr);
+    cudaError_t e = cudaStreamCreateWithFlags(&s_up, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s_dn, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_dn, cudaEventDisableTiming);
+    for (int j = 0; j < nchunk && e == cudaSuccess; ++j) e = cudaEventCreateWithFlags(&ev_up[j], cudaEventDisableTiming);
+    for (int i = 0; i < nslab && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&ev_done[i], cudaEventDisableTiming);
+    const size_t plane = (size_t)p.stride[2];
+    // the workspace may still be in use by earlier work on the caller's stream
+    if (e == cudaSuccess) e = cudaEventRecord(ev_start, st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_up, ev_start, 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_dn, ev_start, 0);
+    struct Arr { const double* h; double* d; int nf; };
+    const Arr in[3] = {{prim_host, d_prim, 8}, {metric_host, d_met, 10}, {K_host, d_K, 6}};
+    int uploaded = 0;   // chunks enqueued so far
+    auto upload_to = [&](int last_chunk) {
+        for (; uploaded <= last_chunk && uploaded < nchunk && e == cudaSuccess; ++uploaded) {
+            const int z0 = uploaded * CH, z1 = (z0 + CH < Nz) ? z0 + CH : Nz;
+            const size_t off = (size_t)z0 * plane, bytes = (size_t)(z1 - z0) * plane * sizeof(double);
+            for (int a = 0; a < 3 && e == cudaSuccess; ++a)
+                for (int bf = 0; bf < p.nbox * in[a].nf && e == cudaSuccess; ++bf)
+                    e = cudaMemcpyAsync(in[a].d + (size_t)bf * p.nc + off, in[a].h + (size_t)bf * p.nc + off, bytes,
+                                        cudaMemcpyHostToDevice, s_up);
+            if (e == cudaSuccess) e = cudaEventRecord(ev_up[uploaded], s_up);
+        }
+    };
+    for (int i = 0; i < nslab && e == cudaSuccess; ++i) {
+        const int k0 = i * CH, k1 = (i == nslab - 1) ? nz : k0 + CH;
+        const int need = (k1 + 2 * g - 1) / CH;                   // last chunk this slab reads
+        upload_to(need + 1);                                      // keep one chunk of upload ahead of the kernels
+        if (e != cudaSuccess) break;
+        e = cudaStreamWaitEvent(st, ev_up[need < nchunk ? need : nchunk - 1], 0);
+        if (e != cudaSuccess) break;
+        grx::RhsParams ps = p;
+        const size_t off = (size_t)k0 * plane;
+        ps.prim = d_prim + off; ps.met = d_met + off; ps.K = d_K + off; ps.out = d_out + off;
+        ps.n[2] = k1 - k0;
+        ps.N[2] = (k1 - k0) + 2 * g;
+        e = launch_variant(ps, recon, st);
+        if (e == cudaSuccess) e = cudaEventRecord(ev_done[i], st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s_dn, ev_done[i], 0);
+        const size_t ooff = (size_t)(k0 + g) * plane, obytes = (size_t)(k1 - k0) * plane * sizeof(double);
+        for (int bf = 0; bf < p.nbox * 8 && e == cudaSuccess; ++bf)
+            e = cudaMemcpyAsync(out_host + (size_t)bf * p.nc + ooff, d_out + (size_t)bf * p.nc + ooff, obytes,
+                                cudaMemcpyDeviceToHost, s_dn);
+    }
+    upload_to(nchunk - 1);
+    // the caller's stream is done when the last download is
+    if (e == cudaSuccess) e = cudaEventRecord(ev_dn, s_dn);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_dn, 0);
+    if (e == cudaSuccess) e = cudaEventRecord(ev_dn, s_up);      // and the (already drained) upload stream
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_dn, 0);
+    for (cudaEvent_t ev : ev_up) if (ev) cudaEventDestroy(ev);
+    for (cudaEvent_t ev : ev_done) if (ev) cudaEventDestroy(ev);
+    if (ev_start) cudaEventDestroy(ev_start);
+    if (ev_dn) cudaEventDestroy(ev_dn);
+    if (s_up) cudaStreamDestroy(s_up);      // destruction is deferred by the runtime until the queued work is done
+    if (s_dn) cudaStreamDestroy(s_dn);
+    if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_host pipeline");
     return GRX_OK;
 }
 

@@ -370,6 +370,30 @@ def test_host_entry_point(grx, oracle):
     assert np.array_equal(ho.numpy()[ii], dev[ii])
 
 
+@pytest.mark.parametrize("n,nbox", [((20, 13, 70), 2), ((9, 6, 33), 1), ((12, 12, 96), 1)])
+def test_host_entry_point_pipelined(grx, oracle, n, nbox):
+    """Blocks with more than 32 planes go through the slab pipeline of grx_valencia_rhs_host (uploads, kernels
+    and downloads of 32-plane slabs overlapped on three streams): same bits as the device entry point, parity
+    with the oracle, ghost cells of the host `out` untouched."""
+    import torch
+    prob = inputs.general_metric_box(n=n, seed=17, nbox=nbox)
+    hp, hm, hk = (torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (prob.prim, prob.metric, prob.K))
+    ws = torch.empty(grx.host_workspace_bytes(hp.shape, prob.nghost) // 8, dtype=torch.float64, device="cuda")
+    for recon in ("weno5", "minmod"):
+        ho = torch.full(hp.shape, -7.25e300, dtype=torch.float64).pin_memory()
+        for _ in range(2):      # twice: the second call reuses the workspace while the first may still be draining
+            grx.valencia_rhs_host(hp, hm, hk, prob.dx, prob.nghost, recon, prob.gamma, ho, ws)
+        torch.cuda.synchronize()
+        got = ho.numpy()
+        dev = gpu_rhs(grx, prob, recon)
+        ii = prob.interior
+        assert np.array_equal(got[ii], dev[ii])
+        ref, _ = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, prob.nghost, recon, prob.gamma)
+        assert relerr_per_component(got[ii], ref[ii]).max() <= TOL
+        g = prob.nghost     # whole interior PLANES come back: the z ghost planes of the host array stay untouched
+        assert np.all(got[:, :, :g] == -7.25e300) and np.all(got[:, :, -g:] == -7.25e300)
+
+
 def test_invalid_arguments_rejected(grx):
     import torch
     prob = inputs.general_metric_box(n=(8, 8, 8), seed=1)
