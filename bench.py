@@ -203,10 +203,26 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------ GPU arm
-def load_workload(name, rank):
+def max_over_ranks(seconds, world, device):
+    """Time of the slowest rank (the contract's `max over ranks`); an all-reduce only when there are ranks."""
+    if world == 1:
+        return float(seconds)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(cells_per_rank, world, steps, t_max):
+    """Weak scaling: every rank evaluates its own block(s); the job's rate counts all of them."""
+    return cells_per_rank * world * steps / t_max
+
+
+def load_workload(name, rank, nbox=None):
     if name.startswith("c5-"):
         N = int(name[3:])
-        nbox = dict(inputs.SWEEP).get(N, 1)
+        nbox = nbox or dict(inputs.SWEEP).get(N, 1)
         if rank == 0:
             return inputs.sweep_boxes(N, nbox)
         # other ranks: same shapes, their own seeds (boxes rank*nbox .. rank*nbox+nbox-1 of the same family)
@@ -297,11 +313,8 @@ def run_ours(args):
         c2 = cs2.summary()
         c2["note"] = "sampled over an untimed repeat of the timed kernel (timed region shorter than the NVML period)"
         clocks = c2
-    tt = torch.tensor([t_dev], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_max = float(tt.item())
-    value = cells * world * args.steps / t_max
+    t_max = max_over_ranks(t_dev, world, "cuda")
+    value = whole_job_rate(cells, world, args.steps, t_max)
 
     # ---- end to end through grx_valencia_rhs_host: pinned host buffers, H2D + kernel + D2H per step
     e2e_steps = max(1, min(args.steps, 5))
@@ -316,10 +329,7 @@ def run_ours(args):
         grx.valencia_rhs_host(hp, hm, hk, prob.dx, g, recon, prob.gamma, ho, ws, stream=stream)
     e1.record(stream)
     stream.synchronize()
-    te = torch.tensor([e0.elapsed_time(e1) * 1e-3], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = cells * world * e2e_steps / float(te.item())
+    e2e_value = whole_job_rate(cells, world, e2e_steps, max_over_ranks(e0.elapsed_time(e1) * 1e-3, world, "cuda"))
     e2e_ok = bool(np.array_equal(ho.numpy()[prob.interior], out.cpu().numpy()[prob.interior]))
     h2d = int(sum(t.numel() for t in (hp, hm, hk)) * 8)
     d2h = int(ho.numel() * 8)
