@@ -41,7 +41,7 @@ UNIT = "cell-updates/s"
 # Algorithmic flops per cell-update of a cubic N^3 box = A + B/N: the operation count of the oracle's
 # counting instance (add = mul = div = sqrt = 1, an FMA would be 2; every face once), fitted on
 # N = 16, 32, 48 general-metric boxes (oracle/count_flops.py; tests/test_bench_model.py re-checks it).
-FLOPS_MODEL = {"weno5": (4753.0, 6209.0), "minmod": (2545.0, 1793.0), "mc": (2640.0, 1500.0)}
+FLOPS_MODEL = {"weno5": (4753.0, 6210.0), "minmod": (2545.0, 1794.0), "mc": (2642.0, 1460.0)}
 # Nominal FP64 peak of a B200: 148 SMs x 64 FP64 lanes x 2 flop (FMA) x 1.965 GHz.
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 KERNEL_OF_VARIANT = {"fused": "rhs_fused_kernel", "staged": "rhs_staged_kernel", "simple": "rhs_simple_kernel",
