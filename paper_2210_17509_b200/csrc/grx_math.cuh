@@ -149,7 +149,8 @@ GRX_HD void face_geom_complete(FaceGeom& m) {
 // ---- a3-a5: one side of a face: admissibility, conserved state, flux, fast speeds -------------------------
 // P: reconstructed primitives of this side; cen[q * nc]: centre values of its donor cell, read only if the
 // side takes the first-order fallback (R5).
-// Returns U (Eqs. 6-9, l.88-94), F^D (Eq. 12, l.108) and the two characteristic speeds (R8).
+// Returns U (Eqs. 6-9, l.88-94) and F^D (Eq. 12, l.108), both WITHOUT their common factor sqrt(gamma), and the two
+// characteristic speeds (R8).
 template <int D>
 GRX_HD void side_state(const double Pin[8], const double* __restrict__ cen, long long nc, const FaceGeom& m,
                        double gamma, double U[8], double F[8], double& lam_m, double& lam_p, unsigned& nfallback) {
@@ -189,14 +190,14 @@ GRX_HD void side_state(const double Pin[8], const double* __restrict__ cen, long
     const double rhohs = rhoh + b2;                          // rho h*
     const double Ps = fma(0.5, b2, p);                       // P*
     const double X = rhohs * W2;
-    const double sg = m.sg;
-    const double Dd = sg * rho * W;                          // Eq. (6)
-    const double Sx = sg * fma(X, vlx, -ab0 * blx);          // Eq. (7)
-    const double Sy = sg * fma(X, vly, -ab0 * bly);
-    const double Sz = sg * fma(X, vlz, -ab0 * blz);
-    const double tau = fma(sg, fma(-ab0, ab0, X - Ps), -Dd); // Eq. (8)
-    const double cBx = sg * Bx, cBy = sg * By, cBz = sg * Bz;  // Eq. (9)
-    U[0] = Dd; U[1] = Sx; U[2] = Sy; U[3] = Sz; U[4] = tau; U[5] = cBx; U[6] = cBy; U[7] = cBz;
+    // sqrt(gamma) is common to both sides of a face and to U and F: it is left out here (U, F are the
+    // UNDENSITISED state and flux) and rides on the HLLE coefficients in face_flux.
+    const double Dd = rho * W;                               // Eq. (6) / sqrt(gamma)
+    const double Sx = fma(X, vlx, -ab0 * blx);               // Eq. (7) / sqrt(gamma)
+    const double Sy = fma(X, vly, -ab0 * bly);
+    const double Sz = fma(X, vlz, -ab0 * blz);
+    const double tau = fma(-ab0, ab0, X - Ps) - Dd;          // Eq. (8) / sqrt(gamma)
+    U[0] = Dd; U[1] = Sx; U[2] = Sy; U[3] = Sz; U[4] = tau; U[5] = Bx; U[6] = By; U[7] = Bz;   // Eq. (9)
     // flux, Eq. (12): vtilde^i = v^i - beta^i/alpha (l.114); everything carries one factor alpha
     const double alp = m.alp;
     const double avx = fma(alp, vx, -m.beta[0]);             // alpha vtilde^i
@@ -204,18 +205,18 @@ GRX_HD void side_state(const double Pin[8], const double* __restrict__ cen, long
     const double avz = fma(alp, vz, -m.beta[2]);
     const double vd = (D == 0) ? vx : (D == 1) ? vy : vz;
     const double avd = (D == 0) ? avx : (D == 1) ? avy : avz;
-    const double cBd = (D == 0) ? cBx : (D == 1) ? cBy : cBz;
-    const double aBdW = alp * cBd * iW;                      // alpha calB^d / W
-    const double asgPs = alp * sg * Ps;
+    const double Bd = (D == 0) ? Bx : (D == 1) ? By : Bz;
+    const double aBdW = alp * Bd * iW;                       // alpha B^d / W
+    const double aPs = alp * Ps;
     F[0] = Dd * avd;
     F[1] = fma(Sx, avd, -blx * aBdW);
     F[2] = fma(Sy, avd, -bly * aBdW);
     F[3] = fma(Sz, avd, -blz * aBdW);
-    F[1 + D] += asgPs;
-    F[4] = fma(tau, avd, fma(asgPs, vd, -ab0 * aBdW));
-    F[5] = fma(cBx, avd, -cBd * avx);
-    F[6] = fma(cBy, avd, -cBd * avy);
-    F[7] = fma(cBz, avd, -cBd * avz);
+    F[1 + D] += aPs;
+    F[4] = fma(tau, avd, fma(aPs, vd, -ab0 * aBdW));
+    F[5] = fma(Bx, avd, -Bd * avx);
+    F[6] = fma(By, avd, -Bd * avy);
+    F[7] = fma(Bz, avd, -Bd * avz);
     F[5 + D] = 0.0;
     // fast-magnetosonic speeds (R8).  With N = b^2 + Gamma p, M = rho h - Gamma p, rho h* = N + M:
     //   a^2 = N/(rho h*), 1 - a^2 = M/(rho h*), 1 - v^2 a^2 = Dn/(rho h*) with Dn = rho h* - v^2 N, so
@@ -247,7 +248,7 @@ GRX_HD void face_flux(FaceGeom& m, const double PL[8], const double PR[8], const
     side_state<D>(PR, cenR, nc, m, gamma, UR, FR, lmR, lpR, nfallback);
     const double lm = fmin(0.0, fmin(lmL, lmR));
     const double lp = fmax(0.0, fmax(lpL, lpR));
-    const double idl = rcp(lp - lm) * scale;      // `scale` (1/dx_d) rides on the three HLLE coefficients
+    const double idl = rcp(lp - lm) * (scale * m.sg);   // 1/dx_d and sqrt(gamma) ride on the three HLLE coefficients
     const double cL = lp * idl, cR = -lm * idl, cU = lp * lm * idl;
 #pragma unroll
     for (int c = 0; c < 8; ++c) Fh[c] = fma(cL, FL[c], fma(cR, FR[c], cU * (UR[c] - UL[c])));

@@ -52,7 +52,7 @@ __device__ __forceinline__ void face_parked(const double* __restrict__ pL, const
     side_state<D>(PR, pL + s, nc, m, gamma, UR, FR, lmR, lpR, nfb);
     const double lm = fmin(0.0, fmin(lmL, lmR));
     const double lp = fmax(0.0, fmax(lpL, lpR));
-    const double idl = rcp(lp - lm) * scale;
+    const double idl = rcp(lp - lm) * (scale * m.sg);
     const double cL = lp * idl, cR = -lm * idl, cU = lp * lm * idl;
 #pragma unroll
     for (int q = 0; q < 8; ++q) Fh[q] = fma(cL, park[(8 + q) * ST], fma(cR, FR[q], cU * (UR[q] - park[q * ST])));
