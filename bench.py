@@ -44,6 +44,9 @@ UNIT = "cell-updates/s"
 FLOPS_MODEL = {"weno5": (4753.0, 6210.0), "minmod": (2545.0, 1794.0), "mc": (2642.0, 1460.0)}
 # Nominal FP64 peak of a B200: 148 SMs x 64 FP64 lanes x 2 flop (FMA) x 1.965 GHz.
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE rhs_fused_kernel launch, from the `ncu --set full` capture
+# summarised in profiles/r1_ncu_fused.md (3.968 GB + 1.098 GB); null for workloads that were not captured.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"c5-256/weno5": 5.066e9}
 KERNEL_OF_VARIANT = {"fused": "rhs_fused_kernel", "staged": "rhs_staged_kernel", "simple": "rhs_simple_kernel",
                      "split": "rhs_z_kernel + rhs_xy_kernel", "ws": "rhs_ws_kernel"}
 
@@ -359,13 +362,8 @@ def run_ours(args):
                 "frac": ach_gbs / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None},
         "traffic": None,
     }
-    tr = os.path.join(ROOT, "profiles", "traffic_bytes_per_launch.json")
-    if os.path.exists(tr):
-        try:
-            with open(tr) as f:
-                roofline["traffic"] = json.load(f).get(f"{args.workload}/{recon}")
-        except (OSError, ValueError):
-            pass
+    if args.variant == "fused":
+        roofline["traffic"] = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(f"{args.workload}/{recon}")
 
     # ---- the oracle on the host cores, bounded sample of the same workload
     cpu_rate, cpu_t, n1, cores = time_oracle(prob, recon, budget_s=args.cpu_seconds)
