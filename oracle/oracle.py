@@ -45,6 +45,8 @@ def lib():
         L.oracle_hlle.restype = None
         L.oracle_sources_point.argtypes = [dp, dp, dp, dp, C.c_double, dp]
         L.oracle_sources_point.restype = None
+        L.oracle_count_piece.argtypes = [C.c_int, C.c_int, C.c_int, up]
+        L.oracle_count_piece.restype = C.c_int
         L.oracle_weno_eps.restype = C.c_double
         L.oracle_v2max.restype = C.c_double
         _lib = L
@@ -145,6 +147,20 @@ def sources_point(P, met, K, dm, gamma):
     S = np.empty(8)
     lib().oracle_sources_point(_p(P), _p(met), _p(K), _p(dm), gamma, _p(S))
     return S
+
+
+PIECES = {"recon_cell": 0, "face_average": 1, "metric_complete_face": 2, "admissible": 3, "prim2con_point": 4,
+          "flux_point": 5, "wavespeeds_point": 6, "hlle": 7, "metric_complete": 8, "derivative": 9,
+          "sources_point": 10, "flux_difference": 11}
+
+
+def count_piece(piece, d=0, recon="weno5"):
+    """Operations {add, mul, div, sqrt} the counting instance executes in ONE evaluation of a piece of the
+    algorithm (oracle_count_piece); the hand counts in tests/test_bench_model.py pin these."""
+    ops = (C.c_ulonglong * 4)()
+    if lib().oracle_count_piece(PIECES[piece], int(d), RECON[recon], ops):
+        raise ValueError("oracle: invalid argument")
+    return dict(add=ops[0], mul=ops[1], div=ops[2], sqrt=ops[3])
 
 
 def weno_eps():

@@ -668,6 +668,56 @@ void oracle_sources_point(const double P[8], const double met[10], const double 
     sources_point(P, m, K, d3, gamma, S);
 }
 
+// ---- point-level COUNTING entry point (tests/test_bench_model.py pins the operation count of every piece
+// against a hand count, so that the roofline numerator is fixed by something other than this file's own total).
+// piece: 0 recon_cell(recon)  1 face average of the 10 metric fields (O1)  2 metric_complete_face(d)
+//        3 admissible  4 prim2con_point  5 flux_point(d)  6 wavespeeds_point(d)  7 hlle  8 metric_complete
+//        9 one 4th-order derivative (O8)  10 sources_point  11 flux difference of one component (O7)
+// ops[4] = {add/sub, mul, div, sqrt}.  The sample inputs are fixed, smooth and admissible; no arithmetic of the
+// double instance is touched.
+int oracle_count_piece(int piece, int d, int recon, unsigned long long ops[4]) {
+    typedef Counted R;
+    if (!ops || d < 0 || d > 2) return 1;
+    R P[8] = {R(0.7), R(0.2), R(-0.1), R(0.3), R(1.3), R(0.4), R(-0.2), R(0.1)};
+    R Q[8] = {R(0.6), R(0.1), R(-0.2), R(0.2), R(1.1), R(0.3), R(-0.1), R(0.2)};
+    Metric<R> m;
+    m.alp = R(0.9); m.beta[0] = R(0.02); m.beta[1] = R(-0.03); m.beta[2] = R(0.01);
+    const double gv[6] = {1.2, 0.1, -0.05, 1.1, 0.07, 0.95};
+    for (int c = 0; c < 6; ++c) m.g[c] = R(gv[c]);
+    metric_complete(m);
+    State<R> s, s2;
+    prim2con_point(P, m, R(1.4), s);
+    prim2con_point(Q, m, R(1.4), s2);
+    R F[8], F2[8], lm, lp, lm2, lp2, out[8];
+    flux_point(P, m, s, d, F); wavespeeds_point(P, m, s, d, R(1.4), lm, lp);
+    flux_point(Q, m, s2, d, F2); wavespeeds_point(Q, m, s2, d, R(1.4), lm2, lp2);
+    t_ops = {0, 0, 0, 0};
+    switch (piece) {
+        case 0: { R qm, qp; recon_cell<R>(recon, R(1.0), R(1.3), R(1.7), R(2.0), R(2.6), qm, qp); break; }
+        case 1: { Metric<R> f; f.alp = R(0.5) * (m.alp + m.alp);
+                  for (int i = 0; i < 3; ++i) f.beta[i] = R(0.5) * (m.beta[i] + m.beta[i]);
+                  for (int c = 0; c < 6; ++c) f.g[c] = R(0.5) * (m.g[c] + m.g[c]);
+                  break; }
+        case 2: metric_complete_face(m, d); break;
+        case 3: (void)admissible(P, m); break;
+        case 4: prim2con_point(P, m, R(1.4), s); break;
+        case 5: flux_point(P, m, s, d, F); break;
+        case 6: wavespeeds_point(P, m, s, d, R(1.4), lm, lp); break;
+        case 7: hlle<R>(s.U, F, lm, lp, s2.U, F2, lm2, lp2, out); break;
+        case 8: metric_complete(m); break;
+        case 9: { R v = (R(8.0) * (R(1.1) - R(0.9)) - (R(1.2) - R(0.8))) / (R(12.0) * R(0.1)); (void)v; break; }
+        case 10: { R K[6], dm[3][10], S[8];
+                   for (int c = 0; c < 6; ++c) K[c] = R(0.01 * (c + 1));
+                   for (int a = 0; a < 3; ++a) for (int f = 0; f < 10; ++f) dm[a][f] = R(0.01 * (a + 1) * (f + 1));
+                   sources_point(P, m, K, dm, R(1.4), S); break; }
+        case 11: { R acc = R(0.0); R div = (F[0] - F2[0]) / R(0.1); acc -= div; (void)acc; break; }
+        default: return 1;
+    }
+    ops[0] = t_ops.add; ops[1] = t_ops.mul; ops[2] = t_ops.div; ops[3] = t_ops.sqrt;
+    t_ops = {0, 0, 0, 0};
+    return 0;
+}
+
 double oracle_weno_eps(void) { return WENO_EPS; }
 double oracle_v2max(void) { return V2MAX; }
 

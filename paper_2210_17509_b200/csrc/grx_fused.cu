@@ -22,6 +22,9 @@
 namespace grx {
 
 constexpr int TX = 32;
+#ifndef GRX_ABL
+#define GRX_ABL 0
+#endif
 
 struct TileGeom {
     int ntx, nty, nzc, tz;   // tiles along x, y; z-chunks and their length
@@ -132,6 +135,10 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
             if (active) {
                 // z: reconstruct this cell, close the face below it, finish the cell below
                 double qm[8], qp[8];
+                if (GRX_ABL & 2) {
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) qm[q] = qp[q] = 0.0;
+                } else
                 recon8<RECON>(prim, nc, c, sz, qm, qp);
                 if (kk >= 0) {
                     double Fh[8];
@@ -140,6 +147,10 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                     double qpz[8];
 #pragma unroll
                     for (int q = 0; q < 8; ++q) qpz[q] = zpark[q * ZS];
+                    if (GRX_ABL & 2) {
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) Fh[q] = qpz[q];
+                    } else
                     face8<2>(prim, met, nc, c - sz, c, qpz, qm, gamma, Fh, (kk == 0 && k0 > 0) ? dup : nfb);
                     // F/dz is rounded once and used with both signs, so a uniform state cancels exactly
 #pragma unroll
@@ -159,6 +170,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
             if (kk < 0 || kk >= nk) continue;   // uniform over the CTA
             // x
             double qm[8];
+            if (!(GRX_ABL & 4)) {
             if (active) {
                 double qp[8];
                 recon8<RECON>(prim, nc, c, 1, qm, qp);
@@ -175,12 +187,16 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 for (int q = 0; q < 8; ++q) Fb.v[q][warp][lane] = Fh[q];
             }
             __syncthreads();
+            }
             // y
+            if (!(GRX_ABL & 8)) {
             if (active) {
+                if (!(GRX_ABL & 4)) {
                 GRX_ACC_LOAD
 #pragma unroll
                 for (int q = 0; q < 8; ++q) acc[q] = fma(Fb.v[q][warp][lane] - Fb.v[q][warp][lane + 1], p.idx[0], acc[q]);
                 GRX_ACC_STORE
+                }
                 double qp[8];
                 recon8<RECON>(prim, nc, c, sy, qm, qp);
 #pragma unroll
@@ -196,13 +212,18 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 for (int q = 0; q < 8; ++q) Fb.v[q][warp][lane] = Fh[q];
             }
             __syncthreads();
+            }
             if (active) {
                 GRX_ACC_LOAD
+                if (!(GRX_ABL & 8)) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) acc[q] = fma(Fb.v[q][warp][lane] - Fb.v[q][warp + 1][lane], p.idx[1], acc[q]);
+                }
+                if (!(GRX_ABL & 1)) {
                 double s1, s2, s3, s4;
                 sources_from_global(p, prim, met, Kf, c, s1, s2, s3, s4);
                 acc[1] += s1; acc[2] += s2; acc[3] += s3; acc[4] += s4;
+                }
                 GRX_ACC_STORE
             }
         }
@@ -222,13 +243,13 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
             const long long cp = cbase + sz * (kk + 1);   // tile origin in plane k0+kk
             double yb_qp[8], yt_qm[8], xr_qm[8];
             long long cxr = 0, cyt = 0;
-            if (ycol) {
+            if (!(GRX_ABL & 8) && ycol) {
                 double tmp[8];
                 recon8<RECON>(prim, nc, cp + lane - sy, sy, tmp, yb_qp);
                 cyt = cp + lane + sy * tye;
                 recon8<RECON>(prim, nc, cyt, sy, yt_qm, tmp);
             }
-            if (xl || xr) {
+            if (!(GRX_ABL & 4) && (xl || xr)) {
                 double qm[8], qp[8];
                 cxr = cp + sy * xrow + (xl ? -1 : txe);
                 recon8<RECON>(prim, nc, cxr, 1, qm, qp);
@@ -239,8 +260,8 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) xr_qm[q] = qm[q];
             }
-            __syncthreads();
-            if (xr) {
+            if (!(GRX_ABL & 4)) __syncthreads();
+            if (!(GRX_ABL & 4) && xr) {
                 double PL[8], Fh[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][xrow][txe];
@@ -248,7 +269,8 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][xrow][txe] = Fh[q];
             }
-            __syncthreads();
+            if (!(GRX_ABL & 4)) __syncthreads();
+            if (!(GRX_ABL & 8)) {
             if (ycol) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Qb.v[q][0][lane] = yb_qp[q];
@@ -263,6 +285,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 for (int q = 0; q < 8; ++q) Fb.v[q][tye][lane] = Fh[q];
             }
             __syncthreads();
+            }
         }
     }
     if (p.nfallback && nfb) atomicAdd(p.nfallback, (unsigned long long)nfb);
