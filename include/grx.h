@@ -51,7 +51,7 @@ enum { GRX_OK = 0, GRX_ERR_INVALID_ARG = 1, GRX_ERR_CUDA = 2, GRX_ERR_UNSUPPORTE
  * (profiles/r1_variants.md): SIMPLE = one thread per cell, every thread evaluates its own six faces;
  * SPLIT = two barrier-free kernels (z + sources, then x + y); STAGED = fused with the current plane staged in
  * shared memory by cp.async; WS = fused plus a helper warp group for the source terms. */
-enum { GRX_VARIANT_FUSED = 0, GRX_VARIANT_SIMPLE = 1, GRX_VARIANT_SPLIT = 2, GRX_VARIANT_STAGED = 3, GRX_VARIANT_WS = 4 };
+enum { GRX_VARIANT_FUSED = 0, GRX_VARIANT_SIMPLE = 1, GRX_VARIANT_SPLIT = 2, GRX_VARIANT_STAGED = 3, GRX_VARIANT_WS = 4, GRX_VARIANT_FLUX = 5 };
 
 /* d/dt of the conserved variables on the interior cells of every box.
  *

@@ -2,6 +2,7 @@
 // No torch types, no allocation, no state besides the kernel-variant switch and the debug counter pointer.
 #include <atomic>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -48,6 +49,12 @@ const char* make_geom(const grx_grid* grid, int nghost, grx::RhsParams& p) {
 // Launches the selected kernel variant on a (sub-)block.
 cudaError_t launch_variant(const grx::RhsParams& p, int recon, cudaStream_t st) {
     const int variant = g_variant.load();
+    if (variant == GRX_VARIANT_FLUX) {
+        if (!grx::flux_supported(p)) return cudaErrorNotSupported;
+        int ty = 7;
+        if (const char* e = std::getenv("GRX_FLUX_TY")) ty = std::atoi(e);
+        return grx::launch_rhs_flux(p, recon, ty, st);
+    }
     return (variant == GRX_VARIANT_SIMPLE)   ? grx::launch_rhs_simple(p, recon, st)
            : (variant == GRX_VARIANT_SPLIT)  ? grx::launch_rhs_split(p, recon, st)
            : (variant == GRX_VARIANT_STAGED) ? grx::launch_rhs_staged(p, recon, st)
@@ -245,7 +252,7 @@ int grx_debug_set_fallback_counter(unsigned long long* counter) {
 }
 
 int grx_set_variant(int variant) {
-    if (variant != GRX_VARIANT_FUSED && variant != GRX_VARIANT_SIMPLE && variant != GRX_VARIANT_SPLIT && variant != GRX_VARIANT_STAGED && variant != GRX_VARIANT_WS) return fail(GRX_ERR_INVALID_ARG, "unknown variant");
+    if (variant != GRX_VARIANT_FUSED && variant != GRX_VARIANT_SIMPLE && variant != GRX_VARIANT_SPLIT && variant != GRX_VARIANT_STAGED && variant != GRX_VARIANT_WS && variant != GRX_VARIANT_FLUX) return fail(GRX_ERR_INVALID_ARG, "unknown variant");
     g_variant.store(variant);
     return GRX_OK;
 }

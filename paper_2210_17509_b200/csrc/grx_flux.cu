@@ -1,0 +1,551 @@
+// grx_flux.cu -- the product kernel, second generation: the fused right-hand side (steps 2-4)
+// with every stencil operand served from shared memory.
+//
+// Same decomposition as grx_fused.cu (a CTA owns an in-plane tile of 32 x TY cells and marches along z, one warp
+// per row plus one rim warp, every face flux computed once), but the memory side is explicit:
+//   * the current plane of the 8 primitives with its halo (3 cells for WENO5, 2 for TVD) and of the 10 metric
+//     fields with a 2-cell halo is brought in by TMA (cp.async.bulk.tensor, one elected thread, mbarrier
+//     completion), one plane ahead of its use;  all in-plane stencil reads (x/y reconstruction, face averages,
+//     x/y metric derivatives) are LDS at compile-time offsets from one per-thread base address;
+//   * the z stencil of the primitives lives in a thread-private ring in shared memory (planes k-2, k-1, k+1;
+//     the centre comes from the staged plane, plane k+2 is the only global load of the reconstruction), so a
+//     step touches each primitive plane once;
+//   * what is left on the global path per cell and step: 8 loads of the look-ahead primitive plane, the own-column
+//     metric of the z face and z derivative, K_ij, and the 8 stores of the finished cell.
+// Requires even Nx and 16-byte aligned arrays (TMA global strides); grx_api.cu falls back to grx_fused.cu otherwise.
+#include <cuda.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <mutex>
+
+#include "grx_launch.h"
+
+namespace grx {
+
+namespace {
+
+constexpr int TX = 32;
+#ifndef GRX_FLUX_DBG
+#define GRX_FLUX_DBG 9
+#endif
+
+struct FluxGeom {
+    int ntx, nty, nzc, tz;
+};
+
+constexpr int align16(int x) { return (x + 15) & ~15; }
+
+// Shared-memory layout (in doubles) of one CTA.
+template <int RECON, int TY>
+struct Lay {
+    static constexpr int H = (RECON == RECON_WENO5) ? 3 : 2;              // halo of the staged primitives
+    static constexpr int PW = TX + 2 * H + 2, PR = TY + 2 * H, PF = PW * PR;  // row pitch (+2: see even start), rows, field stride
+    static constexpr int MH = 2;                                          // halo of the staged metric
+    static constexpr int MW = TX + 2 * MH + 2, MR = TY + 2 * MH, MF = MW * MR;
+    static constexpr int NT = TY * 32;                                    // row-warp threads
+    static constexpr int NRING = (RECON == RECON_WENO5) ? 3 : 1;          // z-history planes of the primitives
+    static constexpr int LOOK = H - 1;                                    // look-ahead plane loaded from global
+    static constexpr int EF = (TY + 1) * (TX + 1);                        // field stride of an exchange buffer
+#ifdef GRX_BAR_FIRST
+    static constexpr int o_bar0 = 0;
+    static constexpr int o_ps = 16;
+#else
+    static constexpr int o_ps = 0;
+#endif
+    static constexpr int o_ms = align16(o_ps + 8 * PF);
+    static constexpr int o_zr = align16(o_ms + 10 * MF);
+    static constexpr int o_qc = o_zr + NRING * 8 * NT;
+    static constexpr int o_qb = o_qc + 8 * NT;
+    static constexpr int o_fb = o_qb + 8 * EF;
+#ifdef GRX_BAR_FIRST
+    static constexpr int o_bar = o_bar0;
+    static constexpr int total = align16(o_fb + 8 * EF);
+#else
+    static constexpr int o_bar = align16(o_fb + 8 * EF);
+    static constexpr int total = o_bar + 16;
+#endif
+    static constexpr unsigned ps_bytes = 8u * PF * sizeof(double);
+    static constexpr unsigned ms_bytes = 10u * MF * sizeof(double);
+};
+
+// ---- mbarrier / TMA primitives (PTX) ---------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred P1;\n\t"
+        "GRX_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+        "@P1 bra GRX_DONE;\n\t"
+        "bra GRX_WAIT;\n\t"
+        "GRX_DONE:\n\t"
+        "}" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map, unsigned bar, int c0, int c1, int c2,
+                                            int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::"r"(dst),
+        "l"(reinterpret_cast<unsigned long long>(map)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
+
+// ---- stencil readers on the staged planes ---------------------------------------------------------------------
+// Reconstruct the 8 primitives of the cell at `pb` (field stride PF) along a direction with element stride S.
+template <int RECON, int PF, int S>
+__device__ __forceinline__ void recon8_smem(const double* pb, double qm[8], double qp[8]) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const double* f = pb + q * PF;
+        double a = 0.0, e = 0.0;
+        if (RECON == RECON_WENO5) { a = f[-2 * S]; e = f[2 * S]; }
+        recon_cell<RECON>(a, f[-S], f[0], f[S], e, qm[q], qp[q]);
+    }
+}
+
+// Two-point average of the ten metric fields between the cell at mb - S and the cell at mb (a1).
+template <int MF, int S>
+__device__ __forceinline__ void face_geom_smem(const double* mb, FaceGeom& m) {
+    double v[10];
+#pragma unroll
+    for (int f = 0; f < 10; ++f) v[f] = 0.5 * (mb[f * MF - S] + mb[f * MF]);
+    m.alp = v[0];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) m.beta[a] = v[1 + a];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) m.g[c] = v[4 + c];
+}
+
+template <int MF, int S>
+__device__ __forceinline__ void dmetric_smem(const double* mb, double d[10]) {
+#pragma unroll
+    for (int f = 0; f < 10; ++f) d[f] = d4raw(mb[f * MF - 2 * S], mb[f * MF - S], mb[f * MF + S], mb[f * MF + 2 * S]);
+}
+
+template <int RECON, int TY>
+__global__ void __launch_bounds__((TY + 1) * 32, 1)
+rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __grid_constant__ CUtensorMap tmP,
+                const __grid_constant__ CUtensorMap tmM) {
+    using L = Lay<RECON, TY>;
+    constexpr int H = L::H, PW = L::PW, PF = L::PF, MH = L::MH, MW = L::MW, MF = L::MF, NT = L::NT, EF = L::EF;
+    constexpr int EW = TX + 1;
+    extern __shared__ __align__(1024) double sm[];
+    double* const PS = sm + L::o_ps;
+    double* const MS = sm + L::o_ms;
+    double* const QB = sm + L::o_qb;   // [8][TY+1][33] reconstructed q^+ handed to the neighbour
+    double* const FB = sm + L::o_fb;   // [8][TY+1][33] face fluxes handed to the neighbour
+    const unsigned barP = smem_u32(sm + L::o_bar), barM = barP + 8;
+
+    int t = blockIdx.x;
+    const int tix = t % tg.ntx; t /= tg.ntx;
+    const int tiy = t % tg.nty; t /= tg.nty;
+    const int zc = t;
+    const int box = blockIdx.y;
+    const int X0 = tix * TX, Y0 = tiy * TY, k0 = zc * tg.tz;
+    const int txe = min(TX, p.n[0] - X0), tye = min(TY, p.n[1] - Y0);
+    const int nk = min(tg.tz, p.n[2] - k0);       // planes owned by this CTA
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    const double* __restrict__ prim = p.prim + (long long)box * 8 * p.nc;
+    const double* __restrict__ met = p.met + (long long)box * 10 * p.nc;
+    const double* __restrict__ Kf = p.K + (long long)box * 6 * p.nc;
+    double* __restrict__ out = p.out + (long long)box * 8 * p.nc;
+    const long long nc = p.nc, sy = p.stride[1], sz = p.stride[2];
+    const double gamma = p.gamma;
+    const long long cbase = (X0 + p.g) + sy * (Y0 + p.g) + sz * (k0 - 1 + p.g);   // tile origin, plane k0-1
+    unsigned nfb = 0;
+
+    // TMA coordinates of the tile's staged boxes (x, y; z and the field block follow per plane).  A box must start
+    // on a 16-byte boundary of global memory (measured: an odd FP64 start coordinate raises "illegal instruction"),
+    // so the box starts at the even column at or below the halo and is two columns wider than the halo needs.
+    const int dP = (p.g - H) & 1, dM = (p.g - MH) & 1;
+    const int pcx = X0 + p.g - H - dP, pcy = Y0 + p.g - H, mcx = X0 + p.g - MH - dM, mcy = Y0 + p.g - MH;
+    const bool producer = (threadIdx.x == TY * 32);
+    if (producer) {
+        mbar_init(barP, 1);
+        mbar_init(barM, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+#ifndef GRX_SUB
+#define GRX_SUB 3
+#endif
+    if (producer) {
+        if (GRX_SUB & 1) {
+        mbar_expect_tx(barP, L::ps_bytes);
+        tma_load_4d(smem_u32(PS), &tmP, barP, pcx, pcy, k0 - 1 + p.g, box * 8);
+        }
+        if (GRX_SUB & 2) {
+        mbar_expect_tx(barM, L::ms_bytes);
+        tma_load_4d(smem_u32(MS), &tmM, barM, mcx, mcy, k0 + p.g, box * 10);
+        }
+    }
+
+    if (GRX_FLUX_DBG == 1) {
+        if (GRX_SUB & 1) mbar_wait(barP, 0);
+        if (GRX_SUB & 2) mbar_wait(barM, 0);
+        if (threadIdx.x == 0) out[0] = PS[0] + MS[0];
+        return;
+    }
+    if (warp < TY) {
+        // ------------------------------------------------ row warp: one cell column per thread
+        const bool active = (GRX_FLUX_DBG >= 3) && (lane < txe) && (warp < tye);
+        long long c = cbase + lane + sy * warp;
+        const double* const psb = PS + (H + warp) * PW + (H + dP + lane);     // this cell in the staged primitives
+        const double* const msb = MS + (MH + warp) * MW + (MH + dM + lane);   // ... and in the staged metric
+        double* const zr = sm + L::o_zr + threadIdx.x;                   // z ring: [slot][field][thread]
+        double* const qc = sm + L::o_qc + threadIdx.x;                   // q^+ of the previous plane: [field][thread]
+        double* const qbx = QB + warp * EW + lane;
+        double* const fbx = FB + warp * EW + lane;
+        int h2 = 0, h1 = 1;                                              // ring slots of planes k-2, k-1 (WENO5); slot 2 = k+1
+        double acc[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+        if (active) {
+            // ring for the first step (plane k0-1): planes k0-3, k0-2 | k0 (WENO5), k0-2 (TVD)
+            if (RECON == RECON_WENO5) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    zr[(0 * 8 + q) * NT] = ldg(prim + q * nc + c - 2 * sz);
+                    zr[(1 * 8 + q) * NT] = ldg(prim + q * nc + c - sz);
+                    zr[(2 * 8 + q) * NT] = ldg(prim + q * nc + c + sz);
+                }
+            } else {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) zr[q * NT] = ldg(prim + q * nc + c - sz);
+            }
+        }
+        for (int kk = -1; kk <= nk; ++kk, c += sz) {
+            // ---------------- z: reconstruct this cell, close the face below it, finish the cell below
+            double qn[8];
+            if (active) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) qn[q] = ldg(prim + q * nc + c + L::LOOK * sz);
+            }
+            mbar_wait(barP, (unsigned)(kk + 1) & 1u);
+            if (active) {
+                double qm[8], qp[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const double c0 = psb[q * PF];
+                    if (RECON == RECON_WENO5) {
+                        recon_cell<RECON>(zr[(h2 * 8 + q) * NT], zr[(h1 * 8 + q) * NT], c0, zr[(2 * 8 + q) * NT], qn[q],
+                                          qm[q], qp[q]);
+                        zr[(h2 * 8 + q) * NT] = c0;       // plane k takes the slot of plane k-2
+                        zr[(2 * 8 + q) * NT] = qn[q];     // plane k+2 takes the slot of plane k+1 (next centre: staged)
+                    } else {
+                        recon_cell<RECON>(0.0, zr[q * NT], c0, qn[q], 0.0, qm[q], qp[q]);
+                        zr[q * NT] = c0;
+                    }
+                }
+                if (kk >= 0) {
+                    double Fh[8], qpz[8];
+                    unsigned dup = 0;   // the first face of an inner chunk is the last face of the chunk below: count once
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) qpz[q] = qc[q * NT];
+                    FaceGeom m;
+                    m.alp = 0.5 * (ldg(met + c - sz) + ldg(met + c));
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) m.beta[a] = 0.5 * (ldg(met + (1 + a) * nc + c - sz) + ldg(met + (1 + a) * nc + c));
+#pragma unroll
+                    for (int g6 = 0; g6 < 6; ++g6) m.g[g6] = 0.5 * (ldg(met + (4 + g6) * nc + c - sz) + ldg(met + (4 + g6) * nc + c));
+                    face_flux<2>(m, qpz, qm, prim + c - sz, prim + c, nc, gamma, Fh, (kk == 0 && k0 > 0) ? dup : nfb);
+                    // F/dz is rounded once and used with both signs, so a uniform state cancels exactly
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) Fh[q] = __dmul_rn(Fh[q], p.idx[2]);
+                    if (kk >= 1) {
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) out[q * nc + c - sz] = __dsub_rn(acc[q], Fh[q]);
+                    }
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) acc[q] = Fh[q];
+                }
+#pragma unroll
+                for (int q = 0; q < 8; ++q) qc[q * NT] = qp[q];
+            }
+            if (RECON == RECON_WENO5) { const int tmp = h2; h2 = h1; h1 = tmp; }
+            if (kk < 0 || kk >= nk) {   // uniform over the CTA: no in-plane work on the planes next to the chunk
+                __syncthreads();
+                continue;
+            }
+            // ---------------- x
+            double qm[8];
+            if (active) {
+                double qp[8];
+                recon8_smem<RECON, PF, 1>(psb, qm, qp);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) qbx[q * EF + 1] = qp[q];
+            }
+            __syncthreads();                                   // (1)
+            mbar_wait(barM, (unsigned)kk & 1u);
+            if (active) {
+                double PL[8], Fh[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) PL[q] = qbx[q * EF];
+                FaceGeom m;
+                face_geom_smem<MF, 1>(msb, m);
+                face_flux<0>(m, PL, qm, prim + c - 1, prim + c, nc, gamma, Fh, nfb);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) fbx[q * EF] = Fh[q];
+            }
+            __syncthreads();                                   // (2)
+            // ---------------- y
+            if (active) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) acc[q] = fma(fbx[q * EF] - fbx[q * EF + 1], p.idx[0], acc[q]);
+                double qp[8];
+                recon8_smem<RECON, PF, PW>(psb, qm, qp);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) qbx[q * EF + EW] = qp[q];
+            }
+            __syncthreads();                                   // (3) the staged primitives are free from here on
+            if (active) {
+                double PL[8], Fh[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) PL[q] = qbx[q * EF];
+                FaceGeom m;
+                face_geom_smem<MF, MW>(msb, m);
+                face_flux<1>(m, PL, qm, prim + c - sy, prim + c, nc, gamma, Fh, nfb);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) fbx[q * EF] = Fh[q];
+                // ---------------- sources (a8 + a9): centre primitives from the ring (plane k sits in slot h1 now)
+                SrcState s;
+                {
+                    double P[8], mm[10];
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) P[q] = (RECON == RECON_WENO5) ? zr[(h1 * 8 + q) * NT] : zr[q * NT];
+#pragma unroll
+                    for (int f = 0; f < 10; ++f) mm[f] = msb[f * MF];
+                    sources_prepare(P, mm, gamma, s);
+                }
+                double st;
+                {
+                    double K6[6];
+#pragma unroll
+                    for (int f = 0; f < 6; ++f) K6[f] = ldg(Kf + f * nc + c);
+                    st = sources_K(s, K6);
+                }
+                double d[10];
+#pragma unroll
+                for (int f = 0; f < 10; ++f) {
+                    const double* mp = met + f * nc + c;
+                    d[f] = d4raw(ldg(mp - 2 * sz), ldg(mp - sz), ldg(mp + sz), ldg(mp + 2 * sz));
+                }
+                acc[3] += sources_dir(s, 2, d, p.idx[2] * (1.0 / 12.0), st);
+                dmetric_smem<MF, 1>(msb, d);
+                acc[1] += sources_dir(s, 0, d, p.idx[0] * (1.0 / 12.0), st);
+                dmetric_smem<MF, MW>(msb, d);
+                acc[2] += sources_dir(s, 1, d, p.idx[1] * (1.0 / 12.0), st);
+                acc[4] += st;
+            }
+            __syncthreads();                                   // (4) the staged metric is free from here on
+            if (active) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) acc[q] = fma(fbx[q * EF] - fbx[q * EF + EW], p.idx[1], acc[q]);
+            }
+        }
+    } else {
+        // ------------------------------------------------ rim warp: the tile's edge work, and the TMA producer
+        // x-rim: lane l < tye          -> cell (X0-1,   Y0+l): its q^+ feeds the first face of row l
+        //        lane TY + l, l < tye  -> cell (X0+txe, Y0+l): its q^- and the last face of row l
+        // y-rim: lane l < txe          -> cell (X0+l, Y0-1) [q^+] and cell (X0+l, Y0+tye) [q^-, last face of column l]
+        const bool rimon = (GRX_FLUX_DBG >= 4);
+        const bool xl = rimon && lane < tye;
+        const bool xr = rimon && (TY <= 16) && lane >= TY && (lane - TY) < tye;
+        const int xrow = xl ? lane : lane - TY;
+        const bool ycol = rimon && lane < txe;
+        // a rim face is the first face of the next tile too: only the block's last faces are counted here
+        const bool count_x = (X0 + txe == p.n[0]), count_y = (Y0 + tye == p.n[1]);
+        unsigned dup = 0;
+        // staged positions: x-rim cell of row xrow, y-rim cells of column `lane`
+        const int xcol = xl ? -1 : txe;
+        const double* const px = PS + (H + xrow) * PW + (H + dP + xcol);
+        const double* const mx = MS + (MH + xrow) * MW + (MH + dM + xcol);
+        const double* const pyb = PS + (H - 1) * PW + (H + dP + lane);
+        const double* const pyt = PS + (H + tye) * PW + (H + dP + lane);
+        const double* const myt = MS + (MH + tye) * MW + (MH + dM + lane);
+        for (int kk = -1; kk <= nk; ++kk) {
+            mbar_wait(barP, (unsigned)(kk + 1) & 1u);
+            if (kk < 0 || kk >= nk) {
+                __syncthreads();
+                if (producer && kk < nk) {
+                    mbar_expect_tx(barP, L::ps_bytes);
+                    tma_load_4d(smem_u32(PS), &tmP, barP, pcx, pcy, k0 + kk + 1 + p.g, box * 8);
+                }
+                continue;
+            }
+            const long long cp = cbase + sz * (kk + 1);   // tile origin in plane k0+kk
+            double yb_qp[8], yt_qm[8], xr_qm[8];
+            if (ycol) {
+                double tmp[8];
+                recon8_smem<RECON, PF, PW>(pyb, tmp, yb_qp);
+                recon8_smem<RECON, PF, PW>(pyt, yt_qm, tmp);
+            }
+            if (xl || xr) {
+                double qm[8], qp[8];
+                recon8_smem<RECON, PF, 1>(px, qm, qp);
+                if (xl) {
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) QB[q * EF + xrow * EW] = qp[q];
+                }
+#pragma unroll
+                for (int q = 0; q < 8; ++q) xr_qm[q] = qm[q];
+            }
+            __syncthreads();                                   // (1)
+            mbar_wait(barM, (unsigned)kk & 1u);
+            if (xr) {
+                double PL[8], Fh[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) PL[q] = QB[q * EF + xrow * EW + txe];
+                FaceGeom m;
+                face_geom_smem<MF, 1>(mx, m);
+                const long long cxr = cp + sy * xrow + txe;
+                face_flux<0>(m, PL, xr_qm, prim + cxr - 1, prim + cxr, nc, gamma, Fh, count_x ? nfb : dup);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) FB[q * EF + xrow * EW + txe] = Fh[q];
+            }
+            __syncthreads();                                   // (2)
+            if (ycol) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) QB[q * EF + lane] = yb_qp[q];
+            }
+            __syncthreads();                                   // (3)
+            if (producer) {   // every read of the staged primitives is done: bring in the next plane
+                mbar_expect_tx(barP, L::ps_bytes);
+                tma_load_4d(smem_u32(PS), &tmP, barP, pcx, pcy, k0 + kk + 1 + p.g, box * 8);
+            }
+            if (ycol) {
+                double PL[8], Fh[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) PL[q] = QB[q * EF + tye * EW + lane];
+                FaceGeom m;
+                face_geom_smem<MF, MW>(myt, m);
+                const long long cyt = cp + lane + sy * tye;
+                face_flux<1>(m, PL, yt_qm, prim + cyt - sy, prim + cyt, nc, gamma, Fh, count_y ? nfb : dup);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) FB[q * EF + tye * EW + lane] = Fh[q];
+            }
+            __syncthreads();                                   // (4)
+            if (producer && kk + 1 < nk) {
+                mbar_expect_tx(barM, L::ms_bytes);
+                tma_load_4d(smem_u32(MS), &tmM, barM, mcx, mcy, k0 + kk + 1 + p.g, box * 10);
+            }
+        }
+    }
+    if (p.nfallback && nfb) atomicAdd(p.nfallback, (unsigned long long)nfb);
+}
+
+// ---- host side ------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void* sym = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(sym);
+    });
+    return fn;
+}
+
+// 4-D map [field*box][z][y][x] of an FP64 SoA array with boxes of bx x by x 1 x nf elements.
+bool make_map(CUtensorMap* map, const double* base, const RhsParams& p, int nf, int bx, int by) {
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) return false;
+    const cuuint64_t dims[4] = {(cuuint64_t)p.N[0], (cuuint64_t)p.N[1], (cuuint64_t)p.N[2], (cuuint64_t)nf * p.nbox};
+    const cuuint64_t strides[3] = {(cuuint64_t)p.N[0] * 8, (cuuint64_t)p.stride[2] * 8, (cuuint64_t)p.nc * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1u, (cuuint32_t)nf};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(base), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (std::getenv("GRX_DUMP_MAP")) {
+        std::printf("map rc %d base %p dims %llu %llu %llu %llu strides %llu %llu %llu box %u %u %u %u sizeof %zu align %zu\n", (int)r, (const void*)base,
+                    (unsigned long long)dims[0], (unsigned long long)dims[1], (unsigned long long)dims[2], (unsigned long long)dims[3],
+                    (unsigned long long)strides[0], (unsigned long long)strides[1], (unsigned long long)strides[2], box[0], box[1], box[2], box[3],
+                    sizeof(CUtensorMap), alignof(CUtensorMap));
+        const unsigned long long* w = reinterpret_cast<const unsigned long long*>(map);
+        for (int i = 0; i < 16; ++i) std::printf("%016llx%c", w[i], i % 4 == 3 ? '\n' : ' ');
+    }
+    return r == CUDA_SUCCESS;
+}
+
+// z-chunking: enough CTAs to fill the machine in whole waves, chunks long enough to amortise the two one-sided
+// plane steps at their ends.
+FluxGeom make_tiles(const RhsParams& p, int ty, int slots) {
+    FluxGeom tg;
+    tg.ntx = (p.n[0] + TX - 1) / TX;
+    tg.nty = (p.n[1] + ty - 1) / ty;
+    const long long inplane = (long long)tg.ntx * tg.nty * p.nbox;
+    int best = 1;
+    double best_eff = -1.0;
+    const int maxc = (p.n[2] + 7) / 8;
+    for (int nzc = 1; nzc <= maxc; ++nzc) {
+        const int tz = (p.n[2] + nzc - 1) / nzc;
+        const int real = (p.n[2] + tz - 1) / tz;
+        if (real != nzc) continue;
+        const double waves = (double)(inplane * nzc) / slots;
+        const double fill = waves / (double)(long long)(waves + 0.999999);
+        const double eff = fill * tz / (tz + 0.45);
+        if (eff > best_eff * 1.001) { best_eff = eff; best = nzc; }
+    }
+    tg.tz = (p.n[2] + best - 1) / best;
+    tg.nzc = (p.n[2] + tg.tz - 1) / tg.tz;
+    return tg;
+}
+
+template <int RECON, int TY>
+cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
+    using L = Lay<RECON, TY>;
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    CUtensorMap tmP, tmM;
+    if (!make_map(&tmP, p.prim, p, 8, L::PW, L::PR) || !make_map(&tmM, p.met, p, 10, L::MW, L::MR))
+        return cudaErrorNotSupported;
+    const size_t smem = (size_t)L::total * sizeof(double);
+    // per device and cheap: set on every launch (no cached state, safe with several devices and host threads)
+    e = cudaFuncSetAttribute(rhs_flux_kernel<RECON, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const FluxGeom tg = make_tiles(p, TY, sms);
+    const dim3 grid((unsigned)(tg.ntx * tg.nty * tg.nzc), p.nbox);
+    rhs_flux_kernel<RECON, TY><<<grid, (TY + 1) * 32, smem, st>>>(p, tg, tmP, tmM);
+    return cudaGetLastError();
+}
+
+template <int RECON>
+cudaError_t dispatch(const RhsParams& p, int ty, cudaStream_t st) {
+    if (ty == 7) return launch_one<RECON, 7>(p, st);
+    return cudaErrorInvalidConfiguration;
+}
+
+}  // namespace
+
+bool flux_supported(const RhsParams& p) {
+    // TMA: global strides are multiples of 16 bytes (even Nx) and the arrays are 16-byte aligned
+    if (p.N[0] % 2 != 0) return false;
+    if (((uintptr_t)p.prim | (uintptr_t)p.met) & 15u) return false;
+    return encode_fn() != nullptr;
+}
+
+cudaError_t launch_rhs_flux(const RhsParams& p, int recon, int ty, cudaStream_t st) {
+    if (recon == RECON_WENO5) return dispatch<RECON_WENO5>(p, ty, st);
+    if (recon == RECON_MC) return dispatch<RECON_MC>(p, ty, st);
+    return dispatch<RECON_MINMOD>(p, ty, st);
+}
+
+}  // namespace grx

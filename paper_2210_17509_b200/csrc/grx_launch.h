@@ -12,6 +12,10 @@ cudaError_t launch_rhs_simple(const RhsParams& p, int recon, cudaStream_t st);
 // grx_fused.cu: the product kernel
 cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st);
 
+// grx_flux.cu: the fused kernel with TMA-staged planes and a shared-memory z ring (needs even Nx, 16-byte alignment)
+bool flux_supported(const RhsParams& p);
+cudaError_t launch_rhs_flux(const RhsParams& p, int recon, int ty, cudaStream_t st);
+
 // grx_split.cu: two barrier-free kernels (z + sources, then x + y)
 cudaError_t launch_rhs_split(const RhsParams& p, int recon, cudaStream_t st);
 
