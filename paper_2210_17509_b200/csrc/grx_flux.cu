@@ -26,9 +26,6 @@ namespace grx {
 namespace {
 
 constexpr int TX = 32;
-#ifndef GRX_FLUX_DBG
-#define GRX_FLUX_DBG 9
-#endif
 
 struct FluxGeom {
     int ntx, nty, nzc, tz;
@@ -39,32 +36,23 @@ constexpr int align16(int x) { return (x + 15) & ~15; }
 // Shared-memory layout (in doubles) of one CTA.
 template <int RECON, int TY>
 struct Lay {
-    static constexpr int H = (RECON == RECON_WENO5) ? 3 : 2;              // halo of the staged primitives
-    static constexpr int PW = TX + 2 * H + 2, PR = TY + 2 * H, PF = PW * PR;  // row pitch (+2: see even start), rows, field stride
-    static constexpr int MH = 2;                                          // halo of the staged metric
+    static constexpr int H = (RECON == RECON_WENO5) ? 3 : 2;                  // halo of the staged primitives
+    static constexpr int PW = TX + 2 * H + 2, PR = TY + 2 * H, PF = PW * PR;  // row pitch (+2: even box start), rows, field stride
+    static constexpr int MH = 2;                                              // halo of the staged metric
     static constexpr int MW = TX + 2 * MH + 2, MR = TY + 2 * MH, MF = MW * MR;
-    static constexpr int NT = TY * 32;                                    // row-warp threads
-    static constexpr int NRING = (RECON == RECON_WENO5) ? 3 : 1;          // z-history planes of the primitives
-    static constexpr int LOOK = H - 1;                                    // look-ahead plane loaded from global
-    static constexpr int EF = (TY + 1) * (TX + 1);                        // field stride of an exchange buffer
-#ifdef GRX_BAR_FIRST
-    static constexpr int o_bar0 = 0;
-    static constexpr int o_ps = 16;
-#else
+    static constexpr int NT = TY * 32;                                        // row-warp threads
+    static constexpr int NRING = (RECON == RECON_WENO5) ? 3 : 1;              // z-history planes of the primitives
+    static constexpr int LOOK = H - 1;                                        // look-ahead plane loaded from global
+    static constexpr int EF = (TY + 1) * TX;                                  // field stride of the y exchange buffer
     static constexpr int o_ps = 0;
-#endif
     static constexpr int o_ms = align16(o_ps + 8 * PF);
     static constexpr int o_zr = align16(o_ms + 10 * MF);
     static constexpr int o_qc = o_zr + NRING * 8 * NT;
-    static constexpr int o_qb = o_qc + 8 * NT;
-    static constexpr int o_fb = o_qb + 8 * EF;
-#ifdef GRX_BAR_FIRST
-    static constexpr int o_bar = o_bar0;
-    static constexpr int total = align16(o_fb + 8 * EF);
-#else
-    static constexpr int o_bar = align16(o_fb + 8 * EF);
+    static constexpr int o_qf = o_qc + 8 * NT;
+    static constexpr int o_fx = o_qf + 8 * EF;
+    static constexpr int o_xp = o_fx + 16 * TY;
+    static constexpr int o_bar = align16(o_xp + 16 * TY);
     static constexpr int total = o_bar + 16;
-#endif
     static constexpr unsigned ps_bytes = 8u * PF * sizeof(double);
     static constexpr unsigned ms_bytes = 10u * MF * sizeof(double);
 };
@@ -96,6 +84,8 @@ __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map
         "l"(reinterpret_cast<unsigned long long>(map)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
         : "memory");
 }
+
+__device__ __forceinline__ void prefetch_l2(const double* a) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a)); }
 
 // ---- stencil readers on the staged planes ---------------------------------------------------------------------
 // Reconstruct the 8 primitives of the cell at `pb` (field stride PF) along a direction with element stride S.
@@ -135,12 +125,13 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
                 const __grid_constant__ CUtensorMap tmM) {
     using L = Lay<RECON, TY>;
     constexpr int H = L::H, PW = L::PW, PF = L::PF, MH = L::MH, MW = L::MW, MF = L::MF, NT = L::NT, EF = L::EF;
-    constexpr int EW = TX + 1;
+    constexpr unsigned FULL = 0xffffffffu;
     extern __shared__ __align__(1024) double sm[];
     double* const PS = sm + L::o_ps;
     double* const MS = sm + L::o_ms;
-    double* const QB = sm + L::o_qb;   // [8][TY+1][33] reconstructed q^+ handed to the neighbour
-    double* const FB = sm + L::o_fb;   // [8][TY+1][33] face fluxes handed to the neighbour
+    double* const QF = sm + L::o_qf;   // [8][TY+1][32] y exchange: q^+ of the row below, then that face's flux
+    double* const FX = sm + L::o_fx;   // [2][8][TY] fluxes of the first and the last x face of every row (rim warp)
+    double* const XP = sm + L::o_xp;   // [2][8][TY] what the first / last lane of a row parks until those arrive
     const unsigned barP = smem_u32(sm + L::o_bar), barM = barP + 8;
 
     int t = blockIdx.x;
@@ -174,37 +165,24 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-#ifndef GRX_SUB
-#define GRX_SUB 3
-#endif
     if (producer) {
-        if (GRX_SUB & 1) {
         mbar_expect_tx(barP, L::ps_bytes);
         tma_load_4d(smem_u32(PS), &tmP, barP, pcx, pcy, k0 - 1 + p.g, box * 8);
-        }
-        if (GRX_SUB & 2) {
         mbar_expect_tx(barM, L::ms_bytes);
         tma_load_4d(smem_u32(MS), &tmM, barM, mcx, mcy, k0 + p.g, box * 10);
-        }
     }
 
-    if (GRX_FLUX_DBG == 1) {
-        if (GRX_SUB & 1) mbar_wait(barP, 0);
-        if (GRX_SUB & 2) mbar_wait(barM, 0);
-        if (threadIdx.x == 0) out[0] = PS[0] + MS[0];
-        return;
-    }
     if (warp < TY) {
         // ------------------------------------------------ row warp: one cell column per thread
-        const bool active = (GRX_FLUX_DBG >= 3) && (lane < txe) && (warp < tye);
+        const bool active = (lane < txe) && (warp < tye);
+        const bool first = (lane == 0), last = (lane == txe - 1);
         long long c = cbase + lane + sy * warp;
         const double* const psb = PS + (H + warp) * PW + (H + dP + lane);     // this cell in the staged primitives
         const double* const msb = MS + (MH + warp) * MW + (MH + dM + lane);   // ... and in the staged metric
-        double* const zr = sm + L::o_zr + threadIdx.x;                   // z ring: [slot][field][thread]
-        double* const qc = sm + L::o_qc + threadIdx.x;                   // q^+ of the previous plane: [field][thread]
-        double* const qbx = QB + warp * EW + lane;
-        double* const fbx = FB + warp * EW + lane;
-        int h2 = 0, h1 = 1;                                              // ring slots of planes k-2, k-1 (WENO5); slot 2 = k+1
+        double* const zr = sm + L::o_zr + threadIdx.x;                        // z ring: [slot][field][thread]
+        double* const qc = sm + L::o_qc + threadIdx.x;                        // q^+ of the previous plane: [field][thread]
+        double* const qf = QF + warp * 32 + lane;                             // this cell's low y face in the exchange
+        int h2 = 0, h1 = 1;                                                   // ring slots of planes k-2, k-1 (WENO5); slot 2 = k+1
         double acc[8];
 #pragma unroll
         for (int q = 0; q < 8; ++q) acc[q] = 0.0;
@@ -228,6 +206,17 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
             if (active) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) qn[q] = ldg(prim + q * nc + c + L::LOOK * sz);
+                if (kk + 2 <= nk) {
+                    // first touches of the step after next: bring their lines from HBM into L2 now
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) prefetch_l2(prim + q * nc + c + (L::LOOK + 2) * sz);
+                    if (kk + 2 < nk) {
+#pragma unroll
+                        for (int f = 0; f < 10; ++f) prefetch_l2(met + f * nc + c + 4 * sz);
+#pragma unroll
+                        for (int f = 0; f < 6; ++f) prefetch_l2(Kf + f * nc + c + 2 * sz);
+                    }
+                }
             }
             mbar_wait(barP, (unsigned)(kk + 1) & 1u);
             if (active) {
@@ -275,46 +264,74 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
                 __syncthreads();
                 continue;
             }
-            // ---------------- x
-            double qm[8];
-            if (active) {
-                double qp[8];
-                recon8_smem<RECON, PF, 1>(psb, qm, qp);
+            // ---------------- x: q^+ and the flux move between neighbouring lanes by warp shuffle; the first and the
+            // last face of the row are the rim warp's (FX), and the lanes next to them park their half of the
+            // difference until the first barrier
+            double qm[8], qx[8];
 #pragma unroll
-                for (int q = 0; q < 8; ++q) qbx[q * EF + 1] = qp[q];
-            }
-            __syncthreads();                                   // (1)
+            for (int q = 0; q < 8; ++q) qx[q] = 0.0;
+            if (active) recon8_smem<RECON, PF, 1>(psb, qm, qx);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) qx[q] = __shfl_up_sync(FULL, qx[q], 1);   // q^+ of the cell to the left
             mbar_wait(barM, (unsigned)kk & 1u);
-            if (active) {
-                double PL[8], Fh[8];
+            double Fx[8];
 #pragma unroll
-                for (int q = 0; q < 8; ++q) PL[q] = qbx[q * EF];
+            for (int q = 0; q < 8; ++q) Fx[q] = 0.0;
+            if (active && !first) {
                 FaceGeom m;
                 face_geom_smem<MF, 1>(msb, m);
-                face_flux<0>(m, PL, qm, prim + c - 1, prim + c, nc, gamma, Fh, nfb);
-#pragma unroll
-                for (int q = 0; q < 8; ++q) fbx[q * EF] = Fh[q];
+                face_flux<0>(m, qx, qm, prim + c - 1, prim + c, nc, gamma, Fx, nfb);
             }
-            __syncthreads();                                   // (2)
-            // ---------------- y
+#pragma unroll
+            for (int q = 0; q < 8; ++q) qx[q] = __shfl_down_sync(FULL, Fx[q], 1);   // flux of the high face
             if (active) {
+                if (!first && !last) {
 #pragma unroll
-                for (int q = 0; q < 8; ++q) acc[q] = fma(fbx[q * EF] - fbx[q * EF + 1], p.idx[0], acc[q]);
-                double qp[8];
-                recon8_smem<RECON, PF, PW>(psb, qm, qp);
+                    for (int q = 0; q < 8; ++q) acc[q] = fma(Fx[q] - qx[q], p.idx[0], acc[q]);
+                } else {
+                    if (first) {
 #pragma unroll
-                for (int q = 0; q < 8; ++q) qbx[q * EF + EW] = qp[q];
+                        for (int q = 0; q < 8; ++q) XP[q * TY + warp] = qx[q];
+                    }
+                    if (last) {
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) XP[(8 + q) * TY + warp] = Fx[q];
+                    }
+                }
+                // ---------------- y
+                recon8_smem<RECON, PF, PW>(psb, qm, qx);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) qf[q * EF + 32] = qx[q];
             }
-            __syncthreads();                                   // (3) the staged primitives are free from here on
+            __syncthreads();                                   // (A) the staged primitives are free from here on
             if (active) {
+                if (first || last) {
+                    // x difference of the row's end cells: low face from FX[0] / parked, high face from parked / FX[1]
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) {
+                        const double lo = first ? FX[q * TY + warp] : XP[(8 + q) * TY + warp];
+                        const double hi = last ? FX[(8 + q) * TY + warp] : XP[q * TY + warp];
+                        acc[q] = fma(lo - hi, p.idx[0], acc[q]);
+                    }
+                }
+                // the global loads of the source terms (z stencil of the metric, K_ij) are issued before the y face so
+                // that their latency is covered by it
+                double dz[10], K6[6];
+#pragma unroll
+                for (int f = 0; f < 10; ++f) {
+                    const double* mp = met + f * nc + c;
+                    dz[f] = d4raw(ldg(mp - 2 * sz), ldg(mp - sz), ldg(mp + sz), ldg(mp + 2 * sz));
+                }
+#pragma unroll
+                for (int f = 0; f < 6; ++f) K6[f] = ldg(Kf + f * nc + c);
                 double PL[8], Fh[8];
 #pragma unroll
-                for (int q = 0; q < 8; ++q) PL[q] = qbx[q * EF];
+                for (int q = 0; q < 8; ++q) PL[q] = qf[q * EF];
                 FaceGeom m;
                 face_geom_smem<MF, MW>(msb, m);
                 face_flux<1>(m, PL, qm, prim + c - sy, prim + c, nc, gamma, Fh, nfb);
 #pragma unroll
-                for (int q = 0; q < 8; ++q) fbx[q * EF] = Fh[q];
+                for (int q = 0; q < 8; ++q) qf[q * EF] = Fh[q];
                 // ---------------- sources (a8 + a9): centre primitives from the ring (plane k sits in slot h1 now)
                 SrcState s;
                 {
@@ -325,52 +342,41 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
                     for (int f = 0; f < 10; ++f) mm[f] = msb[f * MF];
                     sources_prepare(P, mm, gamma, s);
                 }
-                double st;
-                {
-                    double K6[6];
-#pragma unroll
-                    for (int f = 0; f < 6; ++f) K6[f] = ldg(Kf + f * nc + c);
-                    st = sources_K(s, K6);
-                }
+                double st = sources_K(s, K6);
+                acc[3] += sources_dir(s, 2, dz, p.idx[2] * (1.0 / 12.0), st);
                 double d[10];
-#pragma unroll
-                for (int f = 0; f < 10; ++f) {
-                    const double* mp = met + f * nc + c;
-                    d[f] = d4raw(ldg(mp - 2 * sz), ldg(mp - sz), ldg(mp + sz), ldg(mp + 2 * sz));
-                }
-                acc[3] += sources_dir(s, 2, d, p.idx[2] * (1.0 / 12.0), st);
                 dmetric_smem<MF, 1>(msb, d);
                 acc[1] += sources_dir(s, 0, d, p.idx[0] * (1.0 / 12.0), st);
                 dmetric_smem<MF, MW>(msb, d);
                 acc[2] += sources_dir(s, 1, d, p.idx[1] * (1.0 / 12.0), st);
                 acc[4] += st;
             }
-            __syncthreads();                                   // (4) the staged metric is free from here on
+            __syncthreads();                                   // (B) the staged metric is free from here on
             if (active) {
 #pragma unroll
-                for (int q = 0; q < 8; ++q) acc[q] = fma(fbx[q * EF] - fbx[q * EF + EW], p.idx[1], acc[q]);
+                for (int q = 0; q < 8; ++q) acc[q] = fma(qf[q * EF] - qf[q * EF + 32], p.idx[1], acc[q]);
             }
         }
     } else {
-        // ------------------------------------------------ rim warp: the tile's edge work, and the TMA producer
-        // x-rim: lane l < tye          -> cell (X0-1,   Y0+l): its q^+ feeds the first face of row l
-        //        lane TY + l, l < tye  -> cell (X0+txe, Y0+l): its q^- and the last face of row l
-        // y-rim: lane l < txe          -> cell (X0+l, Y0-1) [q^+] and cell (X0+l, Y0+tye) [q^-, last face of column l]
-        const bool rimon = (GRX_FLUX_DBG >= 4);
-        const bool xl = rimon && lane < tye;
-        const bool xr = rimon && (TY <= 16) && lane >= TY && (lane - TY) < tye;
+        // ------------------------------------------------ rim warp: the tile's edge faces, and the TMA producer
+        // x-rim: lane l < tye          -> the first face of row l (between cells X0-1 and X0)
+        //        lane TY + l, l < tye  -> the last face of row l  (between cells X0+txe-1 and X0+txe)
+        // y-rim: lane l < txe          -> cell (X0+l, Y0-1) [q^+ for the row warps] and the last face of column l
+        const bool xl = lane < tye;
+        const bool xr = (TY <= 16) && lane >= TY && (lane - TY) < tye;
         const int xrow = xl ? lane : lane - TY;
-        const bool ycol = rimon && lane < txe;
-        // a rim face is the first face of the next tile too: only the block's last faces are counted here
-        const bool count_x = (X0 + txe == p.n[0]), count_y = (Y0 + tye == p.n[1]);
+        const bool ycol = lane < txe;
+        // the last faces are the first faces of the next tile too: they count only at the block's end
+        const bool count_x = xl || (X0 + txe == p.n[0]), count_y = (Y0 + tye == p.n[1]);
         unsigned dup = 0;
-        // staged positions: x-rim cell of row xrow, y-rim cells of column `lane`
-        const int xcol = xl ? -1 : txe;
+        // staged positions: the cell left of the x-rim face of row xrow, the y-rim cells of column `lane`
+        const int xcol = xl ? -1 : txe - 1;
         const double* const px = PS + (H + xrow) * PW + (H + dP + xcol);
-        const double* const mx = MS + (MH + xrow) * MW + (MH + dM + xcol);
+        const double* const mx = MS + (MH + xrow) * MW + (MH + dM + xcol + 1);
         const double* const pyb = PS + (H - 1) * PW + (H + dP + lane);
         const double* const pyt = PS + (H + tye) * PW + (H + dP + lane);
         const double* const myt = MS + (MH + tye) * MW + (MH + dM + lane);
+        double* const fxo = FX + (xl ? 0 : 8 * TY) + xrow;
         for (int kk = -1; kk <= nk; ++kk) {
             mbar_wait(barP, (unsigned)(kk + 1) & 1u);
             if (kk < 0 || kk >= nk) {
@@ -382,41 +388,27 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
                 continue;
             }
             const long long cp = cbase + sz * (kk + 1);   // tile origin in plane k0+kk
-            double yb_qp[8], yt_qm[8], xr_qm[8];
-            if (ycol) {
-                double tmp[8];
-                recon8_smem<RECON, PF, PW>(pyb, tmp, yb_qp);
-                recon8_smem<RECON, PF, PW>(pyt, yt_qm, tmp);
-            }
-            if (xl || xr) {
-                double qm[8], qp[8];
-                recon8_smem<RECON, PF, 1>(px, qm, qp);
-                if (xl) {
-#pragma unroll
-                    for (int q = 0; q < 8; ++q) QB[q * EF + xrow * EW] = qp[q];
-                }
-#pragma unroll
-                for (int q = 0; q < 8; ++q) xr_qm[q] = qm[q];
-            }
-            __syncthreads();                                   // (1)
             mbar_wait(barM, (unsigned)kk & 1u);
-            if (xr) {
-                double PL[8], Fh[8];
-#pragma unroll
-                for (int q = 0; q < 8; ++q) PL[q] = QB[q * EF + xrow * EW + txe];
+            if (xl || xr) {
+                double PL[8], PR[8], tmp[8], Fh[8];
+                recon8_smem<RECON, PF, 1>(px, tmp, PL);
+                recon8_smem<RECON, PF, 1>(px + 1, PR, tmp);
                 FaceGeom m;
                 face_geom_smem<MF, 1>(mx, m);
-                const long long cxr = cp + sy * xrow + txe;
-                face_flux<0>(m, PL, xr_qm, prim + cxr - 1, prim + cxr, nc, gamma, Fh, count_x ? nfb : dup);
+                const long long cxr = cp + sy * xrow + xcol + 1;
+                face_flux<0>(m, PL, PR, prim + cxr - 1, prim + cxr, nc, gamma, Fh, count_x ? nfb : dup);
 #pragma unroll
-                for (int q = 0; q < 8; ++q) FB[q * EF + xrow * EW + txe] = Fh[q];
+                for (int q = 0; q < 8; ++q) fxo[q * TY] = Fh[q];
             }
-            __syncthreads();                                   // (2)
+            double yt_qm[8];
             if (ycol) {
+                double tmp[8], yb_qp[8];
+                recon8_smem<RECON, PF, PW>(pyb, tmp, yb_qp);
 #pragma unroll
-                for (int q = 0; q < 8; ++q) QB[q * EF + lane] = yb_qp[q];
+                for (int q = 0; q < 8; ++q) QF[q * EF + lane] = yb_qp[q];
+                recon8_smem<RECON, PF, PW>(pyt, yt_qm, tmp);
             }
-            __syncthreads();                                   // (3)
+            __syncthreads();                                   // (A)
             if (producer) {   // every read of the staged primitives is done: bring in the next plane
                 mbar_expect_tx(barP, L::ps_bytes);
                 tma_load_4d(smem_u32(PS), &tmP, barP, pcx, pcy, k0 + kk + 1 + p.g, box * 8);
@@ -424,15 +416,15 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
             if (ycol) {
                 double PL[8], Fh[8];
 #pragma unroll
-                for (int q = 0; q < 8; ++q) PL[q] = QB[q * EF + tye * EW + lane];
+                for (int q = 0; q < 8; ++q) PL[q] = QF[q * EF + tye * 32 + lane];
                 FaceGeom m;
                 face_geom_smem<MF, MW>(myt, m);
                 const long long cyt = cp + lane + sy * tye;
                 face_flux<1>(m, PL, yt_qm, prim + cyt - sy, prim + cyt, nc, gamma, Fh, count_y ? nfb : dup);
 #pragma unroll
-                for (int q = 0; q < 8; ++q) FB[q * EF + tye * EW + lane] = Fh[q];
+                for (int q = 0; q < 8; ++q) QF[q * EF + tye * 32 + lane] = Fh[q];
             }
-            __syncthreads();                                   // (4)
+            __syncthreads();                                   // (B)
             if (producer && kk + 1 < nk) {
                 mbar_expect_tx(barM, L::ms_bytes);
                 tma_load_4d(smem_u32(MS), &tmM, barM, mcx, mcy, k0 + kk + 1 + p.g, box * 10);
@@ -530,6 +522,7 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
 template <int RECON>
 cudaError_t dispatch(const RhsParams& p, int ty, cudaStream_t st) {
     if (ty == 7) return launch_one<RECON, 7>(p, st);
+    if (ty == 11) return launch_one<RECON, 11>(p, st);
     return cudaErrorInvalidConfiguration;
 }
 
