@@ -51,7 +51,11 @@ struct Lay {
     static constexpr int o_qf = o_qc + 8 * NT;
     static constexpr int o_fx = o_qf + 8 * EF;
     static constexpr int o_xp = o_fx + 16 * TY;
-    static constexpr int o_bar = align16(o_xp + 16 * TY);
+    // z ring of the metric (own column, planes k-2 .. k+1 by plane index mod 4): only where shared memory allows it
+    // (7 rows: 211 KB in all); the 11-row tile reads the z stencil of the metric from global memory instead
+    static constexpr bool MZ = (TY <= 7);
+    static constexpr int o_mz = o_xp + 16 * TY;
+    static constexpr int o_bar = align16(o_mz + (MZ ? 4 * 10 * NT : 0));
     static constexpr int total = o_bar + 16;
     static constexpr unsigned ps_bytes = 8u * PF * sizeof(double);
     static constexpr unsigned ms_bytes = 10u * MF * sizeof(double);
@@ -85,6 +89,12 @@ __device__ __forceinline__ void tma_load_4d(unsigned dst, const CUtensorMap* map
         : "memory");
 }
 
+__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, int c1, int c2, int c3) {
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global [%0, {%1, %2, %3, %4}];" ::"l"(
+                     reinterpret_cast<unsigned long long>(map)),
+                 "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+                 : "memory");
+}
 __device__ __forceinline__ void prefetch_l2(const double* a) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a)); }
 
 // ---- stencil readers on the staged planes ---------------------------------------------------------------------
@@ -122,7 +132,7 @@ __device__ __forceinline__ void dmetric_smem(const double* mb, double d[10]) {
 template <int RECON, int TY>
 __global__ void __launch_bounds__((TY + 1) * 32, 1)
 rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __grid_constant__ CUtensorMap tmP,
-                const __grid_constant__ CUtensorMap tmM) {
+                const __grid_constant__ CUtensorMap tmM, const __grid_constant__ CUtensorMap tmK) {
     using L = Lay<RECON, TY>;
     constexpr int H = L::H, PW = L::PW, PF = L::PF, MH = L::MH, MW = L::MW, MF = L::MF, NT = L::NT, EF = L::EF;
     constexpr unsigned FULL = 0xffffffffu;
@@ -158,6 +168,7 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
     // so the box starts at the even column at or below the halo and is two columns wider than the halo needs.
     const int dP = (p.g - H) & 1, dM = (p.g - MH) & 1;
     const int pcx = X0 + p.g - H - dP, pcy = Y0 + p.g - H, mcx = X0 + p.g - MH - dM, mcy = Y0 + p.g - MH;
+    const int kcx = X0 + p.g - (p.g & 1);   // K_ij is only prefetched: own columns from the even column down
     const bool producer = (threadIdx.x == TY * 32);
     if (producer) {
         mbar_init(barP, 1);
@@ -170,6 +181,12 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
         tma_load_4d(smem_u32(PS), &tmP, barP, pcx, pcy, k0 - 1 + p.g, box * 8);
         mbar_expect_tx(barM, L::ms_bytes);
         tma_load_4d(smem_u32(MS), &tmM, barM, mcx, mcy, k0 + p.g, box * 10);
+        // L2 prefetch of the planes the first steps load from global memory (later planes: one per step, below)
+        for (int j = 0; j <= 3; ++j) {
+            tma_prefetch_4d(&tmP, pcx, pcy, k0 + j + p.g, box * 8);
+            tma_prefetch_4d(&tmM, mcx, mcy, k0 + j + p.g, box * 10);
+            if (j <= 1) tma_prefetch_4d(&tmK, kcx, mcy + MH, k0 + j + p.g, box * 6);
+        }
     }
 
     if (warp < TY) {
@@ -182,6 +199,7 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
         double* const zr = sm + L::o_zr + threadIdx.x;                        // z ring: [slot][field][thread]
         double* const qc = sm + L::o_qc + threadIdx.x;                        // q^+ of the previous plane: [field][thread]
         double* const qf = QF + warp * 32 + lane;                             // this cell's low y face in the exchange
+        double* const mz = sm + L::o_mz + threadIdx.x;                        // z ring of the metric: [plane & 3][field][thread]
         int h2 = 0, h1 = 1;                                                   // ring slots of planes k-2, k-1 (WENO5); slot 2 = k+1
         double acc[8];
 #pragma unroll
@@ -199,31 +217,43 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
 #pragma unroll
                 for (int q = 0; q < 8; ++q) zr[q * NT] = ldg(prim + q * nc + c - sz);
             }
+            if (L::MZ) {   // metric planes k0-2, k0-1, k0 (ring slot = plane index relative to k0, mod 4)
+#pragma unroll
+                for (int j = -2; j <= 0; ++j)
+#pragma unroll
+                    for (int f = 0; f < 10; ++f) mz[(((j + 4) & 3) * 10 + f) * NT] = ldg(met + f * nc + c + (j + 1) * sz);
+            }
         }
-        for (int kk = -1; kk <= nk; ++kk, c += sz) {
-            // ---------------- z: reconstruct this cell, close the face below it, finish the cell below
-            double qn[8];
-            if (active) {
+        // The global loads of a step -- the look-ahead plane of the primitives and, with the metric ring, metric plane
+        // k+2 and K_ij -- are issued one step ahead, before the last barrier of the step before, so that they are in
+        // flight while the CTA waits there (with 250 registers, 7 rows; with 168 they would be spilled and are issued
+        // where they are used).  The producer's TMA prefetch has pulled their lines into L2 by then.
+        constexpr bool EARLY = (TY <= 7);
+        double qn[8], mn[10], K6[6], dz[10];
+        auto issue_loads = [&](int kn, long long cn) {
+            if (EARLY && kn <= nk) {
 #pragma unroll
-                for (int q = 0; q < 8; ++q) qn[q] = ldg(prim + q * nc + c + L::LOOK * sz);
-                if (kk + 2 <= nk) {
-                    // first touches of the step after next: bring their lines from HBM into L2 now
+                for (int q = 0; q < 8; ++q) qn[q] = ldg(prim + q * nc + cn + L::LOOK * sz);
+            }
+            if (L::MZ && kn < nk) {
 #pragma unroll
-                    for (int q = 0; q < 8; ++q) prefetch_l2(prim + q * nc + c + (L::LOOK + 2) * sz);
-                    if (kk + 2 < nk) {
+                for (int f = 0; f < 10; ++f) mn[f] = ldg(met + f * nc + cn + 2 * sz);
+                if (kn >= 0) {
 #pragma unroll
-                        for (int f = 0; f < 10; ++f) prefetch_l2(met + f * nc + c + 4 * sz);
-#pragma unroll
-                        for (int f = 0; f < 6; ++f) prefetch_l2(Kf + f * nc + c + 2 * sz);
-                    }
+                    for (int f = 0; f < 6; ++f) K6[f] = ldg(Kf + f * nc + cn);
                 }
             }
+        };
+        if (active) issue_loads(-1, c);
+        for (int kk = -1; kk <= nk; ++kk, c += sz) {
+            // ---------------- z: reconstruct this cell, close the face below it, finish the cell below
             mbar_wait(barP, (unsigned)(kk + 1) & 1u);
             if (active) {
                 double qm[8], qp[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) {
                     const double c0 = psb[q * PF];
+                    if (!EARLY) qn[q] = ldg(prim + q * nc + c + L::LOOK * sz);
                     if (RECON == RECON_WENO5) {
                         recon_cell<RECON>(zr[(h2 * 8 + q) * NT], zr[(h1 * 8 + q) * NT], c0, zr[(2 * 8 + q) * NT], qn[q],
                                           qm[q], qp[q]);
@@ -240,11 +270,21 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
 #pragma unroll
                     for (int q = 0; q < 8; ++q) qpz[q] = qc[q * NT];
                     FaceGeom m;
-                    m.alp = 0.5 * (ldg(met + c - sz) + ldg(met + c));
+                    if (L::MZ) {
+                        const double* m1 = mz + ((kk + 3) & 3) * 10 * NT;   // plane k-1
+                        const double* m0 = mz + (kk & 3) * 10 * NT;         // plane k
+                        m.alp = 0.5 * (m1[0] + m0[0]);
 #pragma unroll
-                    for (int a = 0; a < 3; ++a) m.beta[a] = 0.5 * (ldg(met + (1 + a) * nc + c - sz) + ldg(met + (1 + a) * nc + c));
+                        for (int a = 0; a < 3; ++a) m.beta[a] = 0.5 * (m1[(1 + a) * NT] + m0[(1 + a) * NT]);
 #pragma unroll
-                    for (int g6 = 0; g6 < 6; ++g6) m.g[g6] = 0.5 * (ldg(met + (4 + g6) * nc + c - sz) + ldg(met + (4 + g6) * nc + c));
+                        for (int g6 = 0; g6 < 6; ++g6) m.g[g6] = 0.5 * (m1[(4 + g6) * NT] + m0[(4 + g6) * NT]);
+                    } else {
+                        m.alp = 0.5 * (ldg(met + c - sz) + ldg(met + c));
+#pragma unroll
+                        for (int a = 0; a < 3; ++a) m.beta[a] = 0.5 * (ldg(met + (1 + a) * nc + c - sz) + ldg(met + (1 + a) * nc + c));
+#pragma unroll
+                        for (int g6 = 0; g6 < 6; ++g6) m.g[g6] = 0.5 * (ldg(met + (4 + g6) * nc + c - sz) + ldg(met + (4 + g6) * nc + c));
+                    }
                     face_flux<2>(m, qpz, qm, prim + c - sz, prim + c, nc, gamma, Fh, (kk == 0 && k0 > 0) ? dup : nfb);
                     // F/dz is rounded once and used with both signs, so a uniform state cancels exactly
 #pragma unroll
@@ -258,9 +298,22 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
                 }
 #pragma unroll
                 for (int q = 0; q < 8; ++q) qc[q * NT] = qp[q];
+                if (L::MZ && kk < nk) {
+                    // z stencil sums of the metric for this cell's sources, then plane k+2 takes the slot of plane k-2
+                    const double* m2 = mz + ((kk + 2) & 3) * 10 * NT;
+                    const double* m1 = mz + ((kk + 3) & 3) * 10 * NT;
+                    const double* p1 = mz + ((kk + 1) & 3) * 10 * NT;
+                    if (kk >= 0) {
+#pragma unroll
+                        for (int f = 0; f < 10; ++f) dz[f] = d4raw(m2[f * NT], m1[f * NT], p1[f * NT], mn[f]);
+                    }
+#pragma unroll
+                    for (int f = 0; f < 10; ++f) mz[(((kk + 2) & 3) * 10 + f) * NT] = mn[f];
+                }
             }
             if (RECON == RECON_WENO5) { const int tmp = h2; h2 = h1; h1 = tmp; }
             if (kk < 0 || kk >= nk) {   // uniform over the CTA: no in-plane work on the planes next to the chunk
+                if (active) issue_loads(kk + 1, c + sz);
                 __syncthreads();
                 continue;
             }
@@ -314,16 +367,37 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
                         acc[q] = fma(lo - hi, p.idx[0], acc[q]);
                     }
                 }
-                // the global loads of the source terms (z stencil of the metric, K_ij) are issued before the y face so
-                // that their latency is covered by it
-                double dz[10], K6[6];
+                // ---------------- sources (a8 + a9) before the y face: their global loads (z stencil of the metric,
+                // K_ij) are issued first and land while the part that reads shared memory runs; centre primitives from
+                // the ring (plane k sits in slot h1 now)
+                {
+                    if (!L::MZ) {
 #pragma unroll
-                for (int f = 0; f < 10; ++f) {
-                    const double* mp = met + f * nc + c;
-                    dz[f] = d4raw(ldg(mp - 2 * sz), ldg(mp - sz), ldg(mp + sz), ldg(mp + 2 * sz));
+                        for (int f = 0; f < 10; ++f) {
+                            const double* mp = met + f * nc + c;
+                            dz[f] = d4raw(ldg(mp - 2 * sz), ldg(mp - sz), ldg(mp + sz), ldg(mp + 2 * sz));
+                        }
+#pragma unroll
+                        for (int f = 0; f < 6; ++f) K6[f] = ldg(Kf + f * nc + c);
+                    }
+                    SrcState s;
+                    {
+                        double P[8], mm[10];
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) P[q] = (RECON == RECON_WENO5) ? zr[(h1 * 8 + q) * NT] : zr[q * NT];
+#pragma unroll
+                        for (int f = 0; f < 10; ++f) mm[f] = msb[f * MF];
+                        sources_prepare(P, mm, gamma, s);
+                    }
+                    double st = 0.0, d[10];
+                    dmetric_smem<MF, 1>(msb, d);
+                    acc[1] += sources_dir(s, 0, d, p.idx[0] * (1.0 / 12.0), st);
+                    dmetric_smem<MF, MW>(msb, d);
+                    acc[2] += sources_dir(s, 1, d, p.idx[1] * (1.0 / 12.0), st);
+                    acc[3] += sources_dir(s, 2, dz, p.idx[2] * (1.0 / 12.0), st);
+                    acc[4] += st + sources_K(s, K6);
                 }
-#pragma unroll
-                for (int f = 0; f < 6; ++f) K6[f] = ldg(Kf + f * nc + c);
+                // ---------------- y face
                 double PL[8], Fh[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) PL[q] = qf[q * EF];
@@ -332,24 +406,7 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
                 face_flux<1>(m, PL, qm, prim + c - sy, prim + c, nc, gamma, Fh, nfb);
 #pragma unroll
                 for (int q = 0; q < 8; ++q) qf[q * EF] = Fh[q];
-                // ---------------- sources (a8 + a9): centre primitives from the ring (plane k sits in slot h1 now)
-                SrcState s;
-                {
-                    double P[8], mm[10];
-#pragma unroll
-                    for (int q = 0; q < 8; ++q) P[q] = (RECON == RECON_WENO5) ? zr[(h1 * 8 + q) * NT] : zr[q * NT];
-#pragma unroll
-                    for (int f = 0; f < 10; ++f) mm[f] = msb[f * MF];
-                    sources_prepare(P, mm, gamma, s);
-                }
-                double st = sources_K(s, K6);
-                acc[3] += sources_dir(s, 2, dz, p.idx[2] * (1.0 / 12.0), st);
-                double d[10];
-                dmetric_smem<MF, 1>(msb, d);
-                acc[1] += sources_dir(s, 0, d, p.idx[0] * (1.0 / 12.0), st);
-                dmetric_smem<MF, MW>(msb, d);
-                acc[2] += sources_dir(s, 1, d, p.idx[1] * (1.0 / 12.0), st);
-                acc[4] += st;
+                issue_loads(kk + 1, c + sz);
             }
             __syncthreads();                                   // (B) the staged metric is free from here on
             if (active) {
@@ -412,6 +469,12 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
             if (producer) {   // every read of the staged primitives is done: bring in the next plane
                 mbar_expect_tx(barP, L::ps_bytes);
                 tma_load_4d(smem_u32(PS), &tmP, barP, pcx, pcy, k0 + kk + 1 + p.g, box * 8);
+                // ... and pull the planes the row warps load from global memory a step later from HBM into L2
+                if (kk + 4 <= nk + 2) {
+                    tma_prefetch_4d(&tmP, pcx, pcy, k0 + kk + 4 + p.g, box * 8);
+                    tma_prefetch_4d(&tmM, mcx, mcy, k0 + kk + 4 + p.g, box * 10);
+                }
+                if (kk + 2 < nk) tma_prefetch_4d(&tmK, kcx, mcy + MH, k0 + kk + 2 + p.g, box * 6);
             }
             if (ycol) {
                 double PL[8], Fh[8];
@@ -506,8 +569,9 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return e;
-    CUtensorMap tmP, tmM;
-    if (!make_map(&tmP, p.prim, p, 8, L::PW, L::PR) || !make_map(&tmM, p.met, p, 10, L::MW, L::MR))
+    CUtensorMap tmP, tmM, tmK;
+    if (!make_map(&tmP, p.prim, p, 8, L::PW, L::PR) || !make_map(&tmM, p.met, p, 10, L::MW, L::MR) ||
+        !make_map(&tmK, p.K, p, 6, TX + 2, TY))
         return cudaErrorNotSupported;
     const size_t smem = (size_t)L::total * sizeof(double);
     // per device and cheap: set on every launch (no cached state, safe with several devices and host threads)
@@ -515,7 +579,7 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     const FluxGeom tg = make_tiles(p, TY, sms);
     const dim3 grid((unsigned)(tg.ntx * tg.nty * tg.nzc), p.nbox);
-    rhs_flux_kernel<RECON, TY><<<grid, (TY + 1) * 32, smem, st>>>(p, tg, tmP, tmM);
+    rhs_flux_kernel<RECON, TY><<<grid, (TY + 1) * 32, smem, st>>>(p, tg, tmP, tmM, tmK);
     return cudaGetLastError();
 }
 
@@ -531,7 +595,7 @@ cudaError_t dispatch(const RhsParams& p, int ty, cudaStream_t st) {
 bool flux_supported(const RhsParams& p) {
     // TMA: global strides are multiples of 16 bytes (even Nx) and the arrays are 16-byte aligned
     if (p.N[0] % 2 != 0) return false;
-    if (((uintptr_t)p.prim | (uintptr_t)p.met) & 15u) return false;
+    if (((uintptr_t)p.prim | (uintptr_t)p.met | (uintptr_t)p.K) & 15u) return false;
     return encode_fn() != nullptr;
 }
 

@@ -83,12 +83,12 @@ GRX_HD void recon_cell(double a, double b, double c, double d, double e, double&
         const double u0 = fma(3.0, D2, -D1);                              // a - 4b + 3c
         const double u1 = D2 + D3;                                        // d - b
         const double u2 = fma(-3.0, D3, D4);                              // 3c - 4d + e
-        // 4*beta_k = 13/3 t_k^2 + u_k^2  (the common factor 4 cancels in the weights; epsilon scaled alike)
-        const double k133 = 13.0 / 3.0;
-        const double B0 = fma(k133 * t0, t0, u0 * u0);
-        const double B1 = fma(k133 * t1, t1, u1 * u1);
-        const double B2 = fma(k133 * t2, t2, u2 * u2);
-        double e0 = B0 + 4.0 * WENO_EPS, e1 = B1 + 4.0 * WENO_EPS, e2 = B2 + 4.0 * WENO_EPS;
+        // 4*beta_k + 4 eps = 13/3 t_k^2 + u_k^2 + 4 eps  (the common factor 4 cancels in the weights; the epsilon rides
+        // on the inner FMA)
+        const double k133 = 13.0 / 3.0, eps4 = 4.0 * WENO_EPS;
+        double e0 = fma(k133 * t0, t0, fma(u0, u0, eps4));
+        double e1 = fma(k133 * t1, t1, fma(u1, u1, eps4));
+        double e2 = fma(k133 * t2, t2, fma(u2, u2, eps4));
         e0 *= e0; e1 *= e1; e2 *= e2;
         // a_k = d_k / e_k  ->  multiply all three by e0 e1 e2 (common denominator, R26)
         const double e01 = e0 * e1, e02 = e0 * e2, e12 = e1 * e2;
@@ -96,13 +96,14 @@ GRX_HD void recon_cell(double a, double b, double c, double d, double e, double&
         // plus side: weights (1,6,3)/10 on (e12, e02, e01)
         const double wp2 = 3.0 * e01;
         const double Sp = e12 + w1 + wp2;
-        // 6 p_k - 6 c in differences
-        const double pp0 = fma(5.0, D2, -2.0 * D1), pp1 = fma(2.0, D3, D2), pp2 = fma(4.0, D3, -D4);
+        // 6 p_k - 6 c in differences: 5 D2 - 2 D1 = 2 u0 - D2,  2 D3 + D2,  4 D3 - D4 = D3 - u2
+        const double pp0 = fma(2.0, u0, -D2), pp1 = fma(2.0, D3, D2), pp2 = D3 - u2;
         const double Np = fma(wp2, pp2, fma(w1, pp1, e12 * pp0));
-        // minus side: mirrored stencil, weights (1,6,3)/10 on (e01, e02, e12)
+        // minus side: mirrored stencil, weights (1,6,3)/10 on (e01, e02, e12):  2 D4 - 5 D3 = 2 u2 + D3,
+        // -(2 D2 + D3),  D1 - 4 D2 = -(u0 + D2)
         const double wm2 = 3.0 * e12;
         const double Sm = e01 + w1 + wm2;
-        const double pm0 = fma(-5.0, D3, 2.0 * D4), pm1 = -fma(2.0, D2, D3), pm2 = fma(-4.0, D2, D1);
+        const double pm0 = fma(2.0, u2, D3), pm1 = -fma(2.0, D2, D3), pm2 = -(u0 + D2);
         const double Nm = fma(wm2, pm2, fma(w1, pm1, e01 * pm0));
         const double r = rcp(Sp * Sm) * (1.0 / 6.0);
         qp = fma(Np, Sm * r, c);
