@@ -9,8 +9,13 @@
  * Conventions shared by every entry point
  * ---------------------------------------
  *  - Every array pointer is a DEVICE pointer to FP64 unless it says HOST.  The caller owns all memory;
- *    the library never allocates, frees or keeps user memory, holds no state between calls, and needs
- *    no workspace.
+ *    the library never allocates, frees or keeps user memory.  grx_valencia_rhs and grx_prim2con need no
+ *    workspace; the host entry point grx_valencia_rhs_host takes one from the caller.
+ *  - State: none between calls, except three debug/plumbing items that are stated where they are declared: the
+ *    process-wide kernel selector (grx_set_variant, default AUTO), the per-thread fallback counter pointer
+ *    (grx_debug_set_fallback_counter) and two per-thread CUDA streams that grx_valencia_rhs_host creates on
+ *    first use.  No environment variable is read.  Entry points may be called from several host threads and on
+ *    several devices (the current device of the calling thread is used).
  *  - Layout: structure of arrays, x fastest, ghost zones included, boxes contiguous:
  *        a[box][field][k][j][i],   i in [0,Nx), j in [0,Ny), k in [0,Nz),   N* = n* + 2*nghost,
  *    interior cell (i,j,k) of the paper's block (l.184) sits at (i+nghost, j+nghost, k+nghost).
@@ -46,12 +51,14 @@ typedef struct {
 enum { GRX_RECON_MINMOD = 0, GRX_RECON_MC = 1, GRX_RECON_WENO5 = 2 };
 enum { GRX_OK = 0, GRX_ERR_INVALID_ARG = 1, GRX_ERR_CUDA = 2, GRX_ERR_UNSUPPORTED = 3 };
 
-/* Kernel variants (grx_set_variant).  GRX_VARIANT_FUSED is the product path.  The others compute the same
- * function along a different traversal and are kept as cross-checks and as measured design alternatives
- * (profiles/r1_variants.md): SIMPLE = one thread per cell, every thread evaluates its own six faces;
- * SPLIT = two barrier-free kernels (z + sources, then x + y); STAGED = fused with the current plane staged in
- * shared memory by cp.async; WS = fused plus a helper warp group for the source terms. */
-enum { GRX_VARIANT_FUSED = 0, GRX_VARIANT_SIMPLE = 1, GRX_VARIANT_SPLIT = 2, GRX_VARIANT_STAGED = 3, GRX_VARIANT_WS = 4, GRX_VARIANT_FLUX = 5 };
+/* Kernel selector (grx_set_variant), a debugging and measurement aid.
+ *   AUTO    the product path: the TMA kernel (csrc/grx_tma.cu: planes staged in shared memory by cp.async.bulk.tensor,
+ *           shared-memory z rings) when the arrays qualify -- Nx = nx + 2 nghost even and prim, metric, K 16-byte
+ *           aligned, as TMA needs 16-byte global strides -- and the LDG kernel otherwise;
+ *   SIMPLE  cross-check traversal: one thread per cell, every thread evaluates its own six faces;
+ *   LDG     always the round-1 kernel (csrc/grx_fused.cu: same decomposition, operands through L1 with __ldg);
+ *   TMA     always the TMA kernel; grx_valencia_rhs returns GRX_ERR_UNSUPPORTED when the arrays do not qualify. */
+enum { GRX_VARIANT_AUTO = 0, GRX_VARIANT_SIMPLE = 1, GRX_VARIANT_LDG = 2, GRX_VARIANT_TMA = 3 };
 
 /* d/dt of the conserved variables on the interior cells of every box.
  *
@@ -74,16 +81,17 @@ enum { GRX_VARIANT_FUSED = 0, GRX_VARIANT_SIMPLE = 1, GRX_VARIANT_SPLIT = 2, GRX
  *   out     [nbox][8][Nz][Ny][Nx]   out.  Interior cells are overwritten; ghost cells are not touched
  *           (R23).  Must not alias an input.
  * Returns GRX_OK, GRX_ERR_INVALID_ARG (null pointer, n < 1, nbox < 1, nghost too small, unknown recon,
- * gamma <= 1, dx <= 0, a box larger than 2^31-1 cells) or GRX_ERR_CUDA. */
+ * gamma <= 1, dx <= 0, a box larger than 2^31-1 cells), GRX_ERR_UNSUPPORTED (only with GRX_VARIANT_TMA forced on
+ * arrays that do not qualify) or GRX_ERR_CUDA. */
 int grx_valencia_rhs(const grx_grid* grid, const double* prim, const double* metric, const double* K,
                      const double dx[3], int nghost, int recon, double gamma, double* out, void* cuda_stream);
 
 /* Same computation for HOST arrays (end-to-end entry point): copies prim, metric and K to the device
  * workspace, evaluates the right-hand side there and copies the result back.  Blocks with more than 32 planes
  * along z are processed as a pipeline of 32-plane slabs: the upload of the next slab, the kernel of the current
- * one and the download of the previous one overlap on three streams (two internal ones, created and destroyed
- * per call, ordered after / before `cuda_stream` by events); the results are bitwise those of the device entry
- * point.  Only the INTERIOR planes of `out_host` are written in that case (all of it, ghosts holding whatever
+ * one and the download of the previous one overlap on three streams (two internal ones per host thread and
+ * device, created on first use and kept, ordered after / before `cuda_stream` by events); the results are bitwise
+ * those of the device entry point.  Only the INTERIOR planes of `out_host` are written in that case (all of it, ghosts holding whatever
  * the workspace held, for blocks of <= 32 planes or while a debug fallback counter is set).  The host arrays
  * have the layout above and should be page-locked for the copies to be asynchronous.
  *   workspace        DEVICE pointer, at least grx_host_workspace_bytes(grid, nghost) bytes, owned by the caller.
@@ -118,7 +126,9 @@ int grx_rk_axpy(const grx_grid* grid, int nghost, double a, const double* x, dou
  * first-order fallback.  NULL switches counting off (the default; counting costs a few atomics). */
 int grx_debug_set_fallback_counter(unsigned long long* counter);
 
-/* Selects the kernel variant used by later grx_valencia_rhs calls of this process (default FUSED). */
+/* Selects the kernel used by later grx_valencia_rhs calls of this PROCESS (default GRX_VARIANT_AUTO).  The path
+ * SURVEY.md section 8(b) sketches for the R5 count, grx_debug_fallback_count(host_out, stream), is provided here as
+ * grx_debug_set_fallback_counter above: a caller-owned device counter, so that counting stays asynchronous. */
 int grx_set_variant(int variant);
 
 /* Accuracy self-test of the division-free reciprocal / rsqrt / sqrt helpers the kernels use:

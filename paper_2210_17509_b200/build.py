@@ -15,7 +15,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgrx.so")
 OBJDIR = os.path.join(ROOT, "build", "grx")
-SOURCES = ["grx_api.cu", "grx_simple.cu", "grx_fused.cu", "grx_flux.cu", "grx_split.cu", "grx_staged.cu", "grx_ws.cu", "grx_support.cu"]
+SOURCES = ["grx_api.cu", "grx_simple.cu", "grx_fused.cu", "grx_tma.cu", "grx_support.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--fmad=true",
@@ -55,10 +55,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or not os.path.exists(LIB) or any(os.path.getmtime(o) > os.path.getmtime(LIB) for o in objs):
         cmd = [NVCC, *ARCH, "-shared", "-o", LIB, *objs, "-cudart", "static"]
         subprocess.run(cmd, check=True)
-    # the standalone micro-benchmark (profiles/r1_microbench.md); not linked into the library
-    mb_src, mb_bin = os.path.join(CSRC, "grx_microbench.cu"), os.path.join(HERE, "grx_microbench")
-    if force or not os.path.exists(mb_bin) or os.path.getmtime(mb_bin) < os.path.getmtime(mb_src):
-        subprocess.run([NVCC, *ARCH, "-O3", "-std=c++17", "-o", mb_bin, mb_src], check=True)
     return LIB
 
 

@@ -1,5 +1,6 @@
 // grx_api.cu -- the C ABI of include/grx.h: argument validation on the host, launch geometry, error mapping.
-// No torch types, no allocation, no state besides the kernel-variant switch and the debug counter pointer.
+// No torch types, no allocation of user memory; state: the kernel selector, the per-thread debug counter pointer and
+// the per-thread streams of the host entry point (include/grx.h, "State").
 #include <atomic>
 #include <cstdio>
 #include <cstdlib>
@@ -13,7 +14,7 @@ namespace {
 
 thread_local char t_err[256] = "";
 thread_local unsigned long long* t_fallback_counter = nullptr;
-std::atomic<int> g_variant{GRX_VARIANT_FUSED};
+std::atomic<int> g_variant{GRX_VARIANT_AUTO};
 
 int fail(int code, const char* msg) {
     std::snprintf(t_err, sizeof(t_err), "%s", msg);
@@ -46,20 +47,45 @@ const char* make_geom(const grx_grid* grid, int nghost, grx::RhsParams& p) {
     return nullptr;
 }
 
-// Launches the selected kernel variant on a (sub-)block.
-cudaError_t launch_variant(const grx::RhsParams& p, int recon, cudaStream_t st) {
+// Launches the selected kernel on a (sub-)block.  `unsupported` is set when the TMA kernel was forced on arrays it
+// cannot take.
+cudaError_t launch_variant(const grx::RhsParams& p, int recon, cudaStream_t st, bool* unsupported = nullptr) {
     const int variant = g_variant.load();
-    if (variant == GRX_VARIANT_FLUX) {
-        if (!grx::flux_supported(p)) return cudaErrorNotSupported;
-        int ty = 7;
-        if (const char* e = std::getenv("GRX_FLUX_TY")) ty = std::atoi(e);
-        return grx::launch_rhs_flux(p, recon, ty, st);
+    if (variant == GRX_VARIANT_SIMPLE) return grx::launch_rhs_simple(p, recon, st);
+    if (variant == GRX_VARIANT_LDG) return grx::launch_rhs_fused(p, recon, st);
+    const bool ok = grx::tma_supported(p);
+    if (variant == GRX_VARIANT_TMA && !ok) {
+        if (unsupported) *unsupported = true;
+        return cudaErrorNotSupported;
     }
-    return (variant == GRX_VARIANT_SIMPLE)   ? grx::launch_rhs_simple(p, recon, st)
-           : (variant == GRX_VARIANT_SPLIT)  ? grx::launch_rhs_split(p, recon, st)
-           : (variant == GRX_VARIANT_STAGED) ? grx::launch_rhs_staged(p, recon, st)
-           : (variant == GRX_VARIANT_WS)     ? grx::launch_rhs_ws(p, recon, st)
-                                             : grx::launch_rhs_fused(p, recon, st);
+    return ok ? grx::launch_rhs_tma(p, recon, 7, st) : grx::launch_rhs_fused(p, recon, st);
+}
+
+// The two internal streams of grx_valencia_rhs_host: one pair per host thread and device, created on first use.
+struct HostStreams {
+    int dev = -1;
+    cudaStream_t up = nullptr, dn = nullptr;
+    ~HostStreams() {
+        // At thread exit the context may already be gone: errors are ignored.
+        if (up) cudaStreamDestroy(up);
+        if (dn) cudaStreamDestroy(dn);
+    }
+};
+cudaError_t host_streams(cudaStream_t* up, cudaStream_t* dn) {
+    thread_local std::vector<HostStreams> pool;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    for (HostStreams& h : pool)
+        if (h.dev == dev) { *up = h.up; *dn = h.dn; return cudaSuccess; }
+    pool.emplace_back();
+    HostStreams& h = pool.back();
+    h.dev = dev;
+    e = cudaStreamCreateWithFlags(&h.up, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h.dn, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { pool.pop_back(); return e; }
+    *up = h.up; *dn = h.dn;
+    return cudaSuccess;
 }
 
 }  // namespace
@@ -86,7 +112,9 @@ int grx_valencia_rhs(const grx_grid* grid, const double* prim, const double* met
     p.gamma = gamma;
     p.nfallback = t_fallback_counter;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const cudaError_t e = launch_variant(p, recon, st);
+    bool unsupported = false;
+    const cudaError_t e = launch_variant(p, recon, st, &unsupported);
+    if (unsupported) return fail(GRX_ERR_UNSUPPORTED, "GRX_VARIANT_TMA needs even nx + 2 nghost and 16-byte aligned arrays");
     if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs launch");
     return GRX_OK;
 }
@@ -149,8 +177,7 @@ int grx_valencia_rhs_host(const grx_grid* grid, const double* prim_host, const d
     // a tail shorter than 8 planes joins the last full slab, so that every slab takes the same tile as the whole block
     const int nchunk = (Nz + CH - 1) / CH, nslab = (nz % CH != 0 && nz % CH < 8) ? nz / CH : (nz + CH - 1) / CH;
     std::vector<cudaEvent_t> ev_up(nchunk, nullptr), ev_done(nslab, nullptr);
-    cudaError_t e = cudaStreamCreateWithFlags(&s_up, cudaStreamNonBlocking);
-    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s_dn, cudaStreamNonBlocking);
+    cudaError_t e = host_streams(&s_up, &s_dn);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_dn, cudaEventDisableTiming);
     for (int j = 0; j < nchunk && e == cudaSuccess; ++j) e = cudaEventCreateWithFlags(&ev_up[j], cudaEventDisableTiming);
@@ -204,8 +231,6 @@ int grx_valencia_rhs_host(const grx_grid* grid, const double* prim_host, const d
     for (cudaEvent_t ev : ev_done) if (ev) cudaEventDestroy(ev);
     if (ev_start) cudaEventDestroy(ev_start);
     if (ev_dn) cudaEventDestroy(ev_dn);
-    if (s_up) cudaStreamDestroy(s_up);      // destruction is deferred by the runtime until the queued work is done
-    if (s_dn) cudaStreamDestroy(s_dn);
     if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_host pipeline");
     return GRX_OK;
 }
@@ -252,7 +277,8 @@ int grx_debug_set_fallback_counter(unsigned long long* counter) {
 }
 
 int grx_set_variant(int variant) {
-    if (variant != GRX_VARIANT_FUSED && variant != GRX_VARIANT_SIMPLE && variant != GRX_VARIANT_SPLIT && variant != GRX_VARIANT_STAGED && variant != GRX_VARIANT_WS && variant != GRX_VARIANT_FLUX) return fail(GRX_ERR_INVALID_ARG, "unknown variant");
+    if (variant != GRX_VARIANT_AUTO && variant != GRX_VARIANT_SIMPLE && variant != GRX_VARIANT_LDG && variant != GRX_VARIANT_TMA)
+        return fail(GRX_ERR_INVALID_ARG, "unknown variant");
     g_variant.store(variant);
     return GRX_OK;
 }

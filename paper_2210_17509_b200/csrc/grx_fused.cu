@@ -1,6 +1,7 @@
-// grx_fused.cu -- the product kernel: reconstruct + HLLE + flux divergence in all three directions and the
-// geometric sources in ONE pass over the block (steps 2-4), every face flux computed
-// exactly once.
+// grx_fused.cu -- the round-1 kernel, kept as the path for the shapes the TMA kernel (grx_tma.cu) cannot take (odd
+// Nx, arrays that are not 16-byte aligned): reconstruct + HLLE + flux divergence in all three directions and the
+// geometric sources in ONE pass over the block (steps 2-4), every face flux computed exactly
+// once, all operands read through L1 with __ldg.
 //
 // Decomposition:
 //   * A CTA owns an in-plane tile of TX x TY cells (TX = 32 = one warp along x, TY warps along y) and
@@ -14,17 +15,11 @@
 //     tile belong to one extra "rim warp" per CTA, whose lanes run along the tile edges.
 //   * Sources: metric derivatives and the 3+1 source terms per cell, added to the same accumulators.
 // Global loads go through L1/L2 (__ldg); lanes run along x, so every load is a contiguous 256 B row segment.
-#include <cstdio>
-#include <cstdlib>
-
 #include "grx_launch.h"
 
 namespace grx {
 
 constexpr int TX = 32;
-#ifndef GRX_ABL
-#define GRX_ABL 0
-#endif
 
 struct TileGeom {
     int ntx, nty, nzc, tz;   // tiles along x, y; z-chunks and their length
@@ -121,24 +116,16 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                     for (int f = 0; f < 6; ++f) prefetch_l1(Kf + f * nc + c);
                 }
-                if (tg.pf & 2) {
+                // plane k+3 of the primitives is read by WENO5 at the next step; TVD never reads it, and at the last
+                // step of the last chunk it would lie past the field when nghost = 2
+                if ((tg.pf & 2) && RECON == RECON_WENO5 && kk + 1 < nk) {
 #pragma unroll
                     for (int q = 0; q < 8; ++q) prefetch_l1(prim + q * nc + c + 3 * sz);
-                }
-                if (tg.pf & 4) {
-#pragma unroll
-                    for (int q = 0; q < 8; ++q) prefetch_l2(prim + q * nc + c + 5 * sz);
-#pragma unroll
-                    for (int f = 0; f < 10; ++f) prefetch_l2(met + f * nc + c + 4 * sz);
                 }
             }
             if (active) {
                 // z: reconstruct this cell, close the face below it, finish the cell below
                 double qm[8], qp[8];
-                if (GRX_ABL & 2) {
-#pragma unroll
-                    for (int q = 0; q < 8; ++q) qm[q] = qp[q] = 0.0;
-                } else
                 recon8<RECON>(prim, nc, c, sz, qm, qp);
                 if (kk >= 0) {
                     double Fh[8];
@@ -147,10 +134,6 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                     double qpz[8];
 #pragma unroll
                     for (int q = 0; q < 8; ++q) qpz[q] = zpark[q * ZS];
-                    if (GRX_ABL & 2) {
-#pragma unroll
-                        for (int q = 0; q < 8; ++q) Fh[q] = qpz[q];
-                    } else
                     face8<2>(prim, met, nc, c - sz, c, qpz, qm, gamma, Fh, (kk == 0 && k0 > 0) ? dup : nfb);
                     // F/dz is rounded once and used with both signs, so a uniform state cancels exactly
 #pragma unroll
@@ -170,7 +153,6 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
             if (kk < 0 || kk >= nk) continue;   // uniform over the CTA
             // x
             double qm[8];
-            if (!(GRX_ABL & 4)) {
             if (active) {
                 double qp[8];
                 recon8<RECON>(prim, nc, c, 1, qm, qp);
@@ -187,16 +169,12 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 for (int q = 0; q < 8; ++q) Fb.v[q][warp][lane] = Fh[q];
             }
             __syncthreads();
-            }
             // y
-            if (!(GRX_ABL & 8)) {
             if (active) {
-                if (!(GRX_ABL & 4)) {
                 GRX_ACC_LOAD
 #pragma unroll
                 for (int q = 0; q < 8; ++q) acc[q] = fma(Fb.v[q][warp][lane] - Fb.v[q][warp][lane + 1], p.idx[0], acc[q]);
                 GRX_ACC_STORE
-                }
                 double qp[8];
                 recon8<RECON>(prim, nc, c, sy, qm, qp);
 #pragma unroll
@@ -212,18 +190,13 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 for (int q = 0; q < 8; ++q) Fb.v[q][warp][lane] = Fh[q];
             }
             __syncthreads();
-            }
             if (active) {
                 GRX_ACC_LOAD
-                if (!(GRX_ABL & 8)) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) acc[q] = fma(Fb.v[q][warp][lane] - Fb.v[q][warp + 1][lane], p.idx[1], acc[q]);
-                }
-                if (!(GRX_ABL & 1)) {
                 double s1, s2, s3, s4;
                 sources_from_global(p, prim, met, Kf, c, s1, s2, s3, s4);
                 acc[1] += s1; acc[2] += s2; acc[3] += s3; acc[4] += s4;
-                }
                 GRX_ACC_STORE
             }
         }
@@ -243,13 +216,13 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
             const long long cp = cbase + sz * (kk + 1);   // tile origin in plane k0+kk
             double yb_qp[8], yt_qm[8], xr_qm[8];
             long long cxr = 0, cyt = 0;
-            if (!(GRX_ABL & 8) && ycol) {
+            if (ycol) {
                 double tmp[8];
                 recon8<RECON>(prim, nc, cp + lane - sy, sy, tmp, yb_qp);
                 cyt = cp + lane + sy * tye;
                 recon8<RECON>(prim, nc, cyt, sy, yt_qm, tmp);
             }
-            if (!(GRX_ABL & 4) && (xl || xr)) {
+            if (xl || xr) {
                 double qm[8], qp[8];
                 cxr = cp + sy * xrow + (xl ? -1 : txe);
                 recon8<RECON>(prim, nc, cxr, 1, qm, qp);
@@ -260,8 +233,8 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) xr_qm[q] = qm[q];
             }
-            if (!(GRX_ABL & 4)) __syncthreads();
-            if (!(GRX_ABL & 4) && xr) {
+            __syncthreads();
+            if (xr) {
                 double PL[8], Fh[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][xrow][txe];
@@ -269,8 +242,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][xrow][txe] = Fh[q];
             }
-            if (!(GRX_ABL & 4)) __syncthreads();
-            if (!(GRX_ABL & 8)) {
+            __syncthreads();
             if (ycol) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Qb.v[q][0][lane] = yb_qp[q];
@@ -285,7 +257,6 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 for (int q = 0; q < 8; ++q) Fb.v[q][tye][lane] = Fh[q];
             }
             __syncthreads();
-            }
         }
     }
     if (p.nfallback && nfb) atomicAdd(p.nfallback, (unsigned long long)nfb);
@@ -293,21 +264,6 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 
 // ---- host side ------------------------------------------------------------------------------------------------
 namespace {
-
-struct Config { int ty, minb; };
-
-// GRX_TILE="<TY>x<MINB>" overrides the default tile (tuning knob; the compiled set is listed in dispatch()).
-// Default: 11 rows (12 warps per SM at 168 registers, fastest on every 3-D block of the sweep); blocks that are
-// thin along z have too few plane steps per CTA to amortise the taller tile and take the 7-row one.
-Config pick_config(const RhsParams& p) {
-    Config c = {11, 1};
-    if (p.n[2] < 8) c.ty = 7;
-    if (const char* e = std::getenv("GRX_TILE")) {
-        int ty = 0, mb = 0;
-        if (std::sscanf(e, "%dx%d", &ty, &mb) == 2) { c.ty = ty; c.minb = mb; }
-    }
-    return c;
-}
 
 // z-chunking: enough CTAs to fill the machine a few times over, chunks long enough to amortise the two
 // one-sided plane steps at their ends.
@@ -330,46 +286,34 @@ TileGeom make_tiles(const RhsParams& p, int ty, int slots) {
     }
     tg.tz = (p.n[2] + best - 1) / best;
     tg.nzc = (p.n[2] + tg.tz - 1) / tg.tz;
+    tg.pf = 3;   // software prefetch of the first-touch lines (profiles/r1_variants.md)
     return tg;
 }
 
+// No cached state: the SM count and the shared-memory opt-in are per device and are queried / set on every launch
+// (both are cheap), so the library works with several devices and from several host threads.
 template <int RECON, int TY, int MINB>
 cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
-    static int sms = 0;
-    if (sms == 0) {
-        int dev = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e != cudaSuccess) return e;
-        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) return e;
-    }
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
     const size_t smem = 2 * sizeof(Exch<TY>) + PARK_SLOTS * (TY + 1) * 32 * sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(rhs_fused_kernel<RECON, TY, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
-    TileGeom tg = make_tiles(p, TY, sms * MINB);
-    static const int pf = [] { const char* e = std::getenv("GRX_PREFETCH"); return e ? std::atoi(e) : 3; }();
-    tg.pf = pf;
+    e = cudaFuncSetAttribute(rhs_fused_kernel<RECON, TY, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const TileGeom tg = make_tiles(p, TY, sms * MINB);
     const dim3 grid((unsigned)(tg.ntx * tg.nty * tg.nzc), p.nbox);
     rhs_fused_kernel<RECON, TY, MINB><<<grid, (TY + 1) * 32, smem, st>>>(p, tg);
     return cudaGetLastError();
 }
 
+// 11 rows (12 warps per SM at 168 registers); blocks that are thin along z have too few plane steps per CTA to
+// amortise the taller tile and take the 7-row one (8 warps, 255 registers).
 template <int RECON>
 cudaError_t dispatch(const RhsParams& p, cudaStream_t st) {
-    const Config c = pick_config(p);
-    // compiled tiles: TY regular warps + 1 rim warp per CTA, MINB CTAs per SM (-> register budget)
-    if (c.ty == 7 && c.minb == 2) return launch_one<RECON, 7, 2>(p, st);     // 2 x 256 threads, 128 regs
-    if (c.ty == 11 && c.minb == 1) return launch_one<RECON, 11, 1>(p, st);   // 384 threads, 168 regs
-    if (c.ty == 5 && c.minb == 2) return launch_one<RECON, 5, 2>(p, st);     // 2 x 192 threads, 168 regs
-    if (c.ty == 15 && c.minb == 1) return launch_one<RECON, 15, 1>(p, st);   // 512 threads, 128 regs
-    if (c.ty == 7 && c.minb == 1) return launch_one<RECON, 7, 1>(p, st);     // 256 threads, 255 regs
-    if (c.ty == 6 && c.minb == 1) return launch_one<RECON, 6, 1>(p, st);     // 224 threads, 255 regs
-    return cudaErrorInvalidConfiguration;
+    if (p.n[2] < 8) return launch_one<RECON, 7, 1>(p, st);
+    return launch_one<RECON, 11, 1>(p, st);
 }
 
 }  // namespace

@@ -9,21 +9,12 @@ namespace grx {
 
 // grx_simple.cu: one thread per cell, every thread evaluates its own six faces (cross-check variant)
 cudaError_t launch_rhs_simple(const RhsParams& p, int recon, cudaStream_t st);
-// grx_fused.cu: the product kernel
+// grx_fused.cu: the round-1 kernel (operands through L1), the path for arrays the TMA kernel cannot take
 cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st);
 
-// grx_flux.cu: the fused kernel with TMA-staged planes and a shared-memory z ring (needs even Nx, 16-byte alignment)
-bool flux_supported(const RhsParams& p);
-cudaError_t launch_rhs_flux(const RhsParams& p, int recon, int ty, cudaStream_t st);
-
-// grx_split.cu: two barrier-free kernels (z + sources, then x + y)
-cudaError_t launch_rhs_split(const RhsParams& p, int recon, cudaStream_t st);
-
-// grx_staged.cu: fused kernel with the current plane staged in shared memory by cp.async
-cudaError_t launch_rhs_staged(const RhsParams& p, int recon, cudaStream_t st);
-
-// grx_ws.cu: fused kernel plus a helper warp group for the sources (setmaxnreg)
-cudaError_t launch_rhs_ws(const RhsParams& p, int recon, cudaStream_t st);
+// grx_tma.cu: the product kernel (TMA-staged planes, shared-memory z rings); needs even Nx and 16-byte aligned arrays
+bool tma_supported(const RhsParams& p);
+cudaError_t launch_rhs_tma(const RhsParams& p, int recon, int ty, cudaStream_t st);
 
 // grx_support.cu
 cudaError_t launch_prim2con(const double* prim, const double* met, long long nc, int nbox, double gamma, double* cons,

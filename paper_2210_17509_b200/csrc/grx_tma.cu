@@ -1,18 +1,22 @@
-// grx_flux.cu -- the product kernel, second generation: the fused right-hand side (steps 2-4)
-// with every stencil operand served from shared memory.
+// grx_tma.cu -- the product kernel: the fused right-hand side (steps 2-4: reconstruct -> HLLE ->
+// flux divergence + sources, all three directions, every face flux computed once) with every stencil operand served
+// from shared memory.
 //
-// Same decomposition as grx_fused.cu (a CTA owns an in-plane tile of 32 x TY cells and marches along z, one warp
-// per row plus one rim warp, every face flux computed once), but the memory side is explicit:
+// Decomposition: a CTA owns an in-plane tile of 32 x TY cells (one warp per row, lanes along x) and marches along z
+// through a chunk of the block, one plane per step; an extra "rim" warp computes the faces on the tile's edge and
+// drives the TMA engine.  The memory side is explicit:
 //   * the current plane of the 8 primitives with its halo (3 cells for WENO5, 2 for TVD) and of the 10 metric
 //     fields with a 2-cell halo is brought in by TMA (cp.async.bulk.tensor, one elected thread, mbarrier
-//     completion), one plane ahead of its use;  all in-plane stencil reads (x/y reconstruction, face averages,
+//     completion), one step ahead of its use; all in-plane stencil reads (x/y reconstruction, face averages,
 //     x/y metric derivatives) are LDS at compile-time offsets from one per-thread base address;
-//   * the z stencil of the primitives lives in a thread-private ring in shared memory (planes k-2, k-1, k+1;
-//     the centre comes from the staged plane, plane k+2 is the only global load of the reconstruction), so a
-//     step touches each primitive plane once;
-//   * what is left on the global path per cell and step: 8 loads of the look-ahead primitive plane, the own-column
-//     metric of the z face and z derivative, K_ij, and the 8 stores of the finished cell.
-// Requires even Nx and 16-byte aligned arrays (TMA global strides); grx_api.cu falls back to grx_fused.cu otherwise.
+//   * the z stencils live in thread-private rings in shared memory: the primitives (planes k-2, k-1, k+1; the centre
+//     comes from the staged plane) and the metric (planes k-2 .. k+1), so a step touches each plane once;
+//   * what is left on the global path per cell and step -- the look-ahead plane of the primitives (8 loads), metric
+//     plane k+2 (10), K_ij (6) -- is loaded one step ahead, before the step's last barrier, from lines the producer has
+//     pulled into L2 with cp.async.bulk.prefetch.tensor; plus the 8 stores of the finished cell;
+//   * x: q^+ and the flux move between neighbouring lanes by warp shuffle; y: one exchange buffer, two barriers per
+//     plane.
+// Requires even Nx and 16-byte aligned arrays (TMA global strides); grx_api.cu takes grx_fused.cu otherwise.
 #include <cuda.h>
 
 #include <cstdio>
@@ -27,7 +31,7 @@ namespace {
 
 constexpr int TX = 32;
 
-struct FluxGeom {
+struct TmaGeom {
     int ntx, nty, nzc, tz;
 };
 
@@ -51,12 +55,10 @@ struct Lay {
     static constexpr int o_qf = o_qc + 8 * NT;
     static constexpr int o_fx = o_qf + 8 * EF;
     static constexpr int o_xp = o_fx + 16 * TY;
-    // z ring of the metric (own column, planes k-2 .. k+1 by plane index mod 4): only where shared memory allows it
-    // (7 rows: 211 KB in all); the 11-row tile reads the z stencil of the metric from global memory instead
-    static constexpr bool MZ = (TY <= 7);
-    static constexpr int o_mz = o_xp + 16 * TY;
-    static constexpr int o_bar = align16(o_mz + (MZ ? 4 * 10 * NT : 0));
+    static constexpr int o_mz = o_xp + 16 * TY;                               // z ring of the metric: planes k-2 .. k+1 by (plane & 3)
+    static constexpr int o_bar = align16(o_mz + 4 * 10 * NT);
     static constexpr int total = o_bar + 16;
+    static_assert(total * sizeof(double) <= 227 * 1024, "tile does not fit the 227 KB of shared memory of a CTA");
     static constexpr unsigned ps_bytes = 8u * PF * sizeof(double);
     static constexpr unsigned ms_bytes = 10u * MF * sizeof(double);
 };
@@ -95,7 +97,6 @@ __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, 
                  "r"(c0), "r"(c1), "r"(c2), "r"(c3)
                  : "memory");
 }
-__device__ __forceinline__ void prefetch_l2(const double* a) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a)); }
 
 // ---- stencil readers on the staged planes ---------------------------------------------------------------------
 // Reconstruct the 8 primitives of the cell at `pb` (field stride PF) along a direction with element stride S.
@@ -131,11 +132,12 @@ __device__ __forceinline__ void dmetric_smem(const double* mb, double d[10]) {
 
 template <int RECON, int TY>
 __global__ void __launch_bounds__((TY + 1) * 32, 1)
-rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __grid_constant__ CUtensorMap tmP,
+rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __grid_constant__ CUtensorMap tmP,
                 const __grid_constant__ CUtensorMap tmM, const __grid_constant__ CUtensorMap tmK) {
     using L = Lay<RECON, TY>;
     constexpr int H = L::H, PW = L::PW, PF = L::PF, MH = L::MH, MW = L::MW, MF = L::MF, NT = L::NT, EF = L::EF;
     constexpr unsigned FULL = 0xffffffffu;
+    static_assert(2 * TY <= 32, "the rim warp needs two lanes per row");
     extern __shared__ __align__(1024) double sm[];
     double* const PS = sm + L::o_ps;
     double* const MS = sm + L::o_ms;
@@ -217,25 +219,22 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
 #pragma unroll
                 for (int q = 0; q < 8; ++q) zr[q * NT] = ldg(prim + q * nc + c - sz);
             }
-            if (L::MZ) {   // metric planes k0-2, k0-1, k0 (ring slot = plane index relative to k0, mod 4)
+            // metric planes k0-2, k0-1, k0 (ring slot = plane index relative to k0, mod 4)
 #pragma unroll
-                for (int j = -2; j <= 0; ++j)
+            for (int j = -2; j <= 0; ++j)
 #pragma unroll
-                    for (int f = 0; f < 10; ++f) mz[(((j + 4) & 3) * 10 + f) * NT] = ldg(met + f * nc + c + (j + 1) * sz);
-            }
+                for (int f = 0; f < 10; ++f) mz[(((j + 4) & 3) * 10 + f) * NT] = ldg(met + f * nc + c + (j + 1) * sz);
         }
-        // The global loads of a step -- the look-ahead plane of the primitives and, with the metric ring, metric plane
-        // k+2 and K_ij -- are issued one step ahead, before the last barrier of the step before, so that they are in
-        // flight while the CTA waits there (with 250 registers, 7 rows; with 168 they would be spilled and are issued
-        // where they are used).  The producer's TMA prefetch has pulled their lines into L2 by then.
-        constexpr bool EARLY = (TY <= 7);
+        // The global loads of a step -- the look-ahead plane of the primitives, metric plane k+2 and K_ij -- are issued
+        // one step ahead, before the last barrier of the step before, so that they are in flight while the CTA waits
+        // there.  The producer's TMA prefetch has pulled their lines into L2 by then.
         double qn[8], mn[10], K6[6], dz[10];
         auto issue_loads = [&](int kn, long long cn) {
-            if (EARLY && kn <= nk) {
+            if (kn <= nk) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) qn[q] = ldg(prim + q * nc + cn + L::LOOK * sz);
             }
-            if (L::MZ && kn < nk) {
+            if (kn < nk) {
 #pragma unroll
                 for (int f = 0; f < 10; ++f) mn[f] = ldg(met + f * nc + cn + 2 * sz);
                 if (kn >= 0) {
@@ -253,7 +252,6 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
 #pragma unroll
                 for (int q = 0; q < 8; ++q) {
                     const double c0 = psb[q * PF];
-                    if (!EARLY) qn[q] = ldg(prim + q * nc + c + L::LOOK * sz);
                     if (RECON == RECON_WENO5) {
                         recon_cell<RECON>(zr[(h2 * 8 + q) * NT], zr[(h1 * 8 + q) * NT], c0, zr[(2 * 8 + q) * NT], qn[q],
                                           qm[q], qp[q]);
@@ -270,7 +268,7 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
 #pragma unroll
                     for (int q = 0; q < 8; ++q) qpz[q] = qc[q * NT];
                     FaceGeom m;
-                    if (L::MZ) {
+                    {
                         const double* m1 = mz + ((kk + 3) & 3) * 10 * NT;   // plane k-1
                         const double* m0 = mz + (kk & 3) * 10 * NT;         // plane k
                         m.alp = 0.5 * (m1[0] + m0[0]);
@@ -278,12 +276,6 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
                         for (int a = 0; a < 3; ++a) m.beta[a] = 0.5 * (m1[(1 + a) * NT] + m0[(1 + a) * NT]);
 #pragma unroll
                         for (int g6 = 0; g6 < 6; ++g6) m.g[g6] = 0.5 * (m1[(4 + g6) * NT] + m0[(4 + g6) * NT]);
-                    } else {
-                        m.alp = 0.5 * (ldg(met + c - sz) + ldg(met + c));
-#pragma unroll
-                        for (int a = 0; a < 3; ++a) m.beta[a] = 0.5 * (ldg(met + (1 + a) * nc + c - sz) + ldg(met + (1 + a) * nc + c));
-#pragma unroll
-                        for (int g6 = 0; g6 < 6; ++g6) m.g[g6] = 0.5 * (ldg(met + (4 + g6) * nc + c - sz) + ldg(met + (4 + g6) * nc + c));
                     }
                     face_flux<2>(m, qpz, qm, prim + c - sz, prim + c, nc, gamma, Fh, (kk == 0 && k0 > 0) ? dup : nfb);
                     // F/dz is rounded once and used with both signs, so a uniform state cancels exactly
@@ -298,7 +290,7 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
                 }
 #pragma unroll
                 for (int q = 0; q < 8; ++q) qc[q * NT] = qp[q];
-                if (L::MZ && kk < nk) {
+                if (kk < nk) {
                     // z stencil sums of the metric for this cell's sources, then plane k+2 takes the slot of plane k-2
                     const double* m2 = mz + ((kk + 2) & 3) * 10 * NT;
                     const double* m1 = mz + ((kk + 3) & 3) * 10 * NT;
@@ -367,19 +359,9 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
                         acc[q] = fma(lo - hi, p.idx[0], acc[q]);
                     }
                 }
-                // ---------------- sources (a8 + a9) before the y face: their global loads (z stencil of the metric,
-                // K_ij) are issued first and land while the part that reads shared memory runs; centre primitives from
-                // the ring (plane k sits in slot h1 now)
+                // ---------------- sources (a8 + a9): centre primitives from the ring (plane k sits in slot h1 now), x and
+                // y stencils of the metric from the staged plane, z stencil sums and K_ij from the top of the step
                 {
-                    if (!L::MZ) {
-#pragma unroll
-                        for (int f = 0; f < 10; ++f) {
-                            const double* mp = met + f * nc + c;
-                            dz[f] = d4raw(ldg(mp - 2 * sz), ldg(mp - sz), ldg(mp + sz), ldg(mp + 2 * sz));
-                        }
-#pragma unroll
-                        for (int f = 0; f < 6; ++f) K6[f] = ldg(Kf + f * nc + c);
-                    }
                     SrcState s;
                     {
                         double P[8], mm[10];
@@ -420,7 +402,7 @@ rhs_flux_kernel(const __grid_constant__ RhsParams p, const FluxGeom tg, const __
         //        lane TY + l, l < tye  -> the last face of row l  (between cells X0+txe-1 and X0+txe)
         // y-rim: lane l < txe          -> cell (X0+l, Y0-1) [q^+ for the row warps] and the last face of column l
         const bool xl = lane < tye;
-        const bool xr = (TY <= 16) && lane >= TY && (lane - TY) < tye;
+        const bool xr = lane >= TY && (lane - TY) < tye;
         const int xrow = xl ? lane : lane - TY;
         const bool ycol = lane < txe;
         // the last faces are the first faces of the next tile too: they count only at the block's end
@@ -526,21 +508,13 @@ bool make_map(CUtensorMap* map, const double* base, const RhsParams& p, int nf, 
     const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(base), dims, strides, box, estr,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (std::getenv("GRX_DUMP_MAP")) {
-        std::printf("map rc %d base %p dims %llu %llu %llu %llu strides %llu %llu %llu box %u %u %u %u sizeof %zu align %zu\n", (int)r, (const void*)base,
-                    (unsigned long long)dims[0], (unsigned long long)dims[1], (unsigned long long)dims[2], (unsigned long long)dims[3],
-                    (unsigned long long)strides[0], (unsigned long long)strides[1], (unsigned long long)strides[2], box[0], box[1], box[2], box[3],
-                    sizeof(CUtensorMap), alignof(CUtensorMap));
-        const unsigned long long* w = reinterpret_cast<const unsigned long long*>(map);
-        for (int i = 0; i < 16; ++i) std::printf("%016llx%c", w[i], i % 4 == 3 ? '\n' : ' ');
-    }
     return r == CUDA_SUCCESS;
 }
 
 // z-chunking: enough CTAs to fill the machine in whole waves, chunks long enough to amortise the two one-sided
 // plane steps at their ends.
-FluxGeom make_tiles(const RhsParams& p, int ty, int slots) {
-    FluxGeom tg;
+TmaGeom make_tiles(const RhsParams& p, int ty, int slots) {
+    TmaGeom tg;
     tg.ntx = (p.n[0] + TX - 1) / TX;
     tg.nty = (p.n[1] + ty - 1) / ty;
     const long long inplane = (long long)tg.ntx * tg.nty * p.nbox;
@@ -575,31 +549,31 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
         return cudaErrorNotSupported;
     const size_t smem = (size_t)L::total * sizeof(double);
     // per device and cheap: set on every launch (no cached state, safe with several devices and host threads)
-    e = cudaFuncSetAttribute(rhs_flux_kernel<RECON, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    e = cudaFuncSetAttribute(rhs_tma_kernel<RECON, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    const FluxGeom tg = make_tiles(p, TY, sms);
+    const TmaGeom tg = make_tiles(p, TY, sms);
     const dim3 grid((unsigned)(tg.ntx * tg.nty * tg.nzc), p.nbox);
-    rhs_flux_kernel<RECON, TY><<<grid, (TY + 1) * 32, smem, st>>>(p, tg, tmP, tmM, tmK);
+    rhs_tma_kernel<RECON, TY><<<grid, (TY + 1) * 32, smem, st>>>(p, tg, tmP, tmM, tmK);
     return cudaGetLastError();
 }
 
 template <int RECON>
 cudaError_t dispatch(const RhsParams& p, int ty, cudaStream_t st) {
+    // 7 rows: 8 warps per SM at 254 registers, 211 KB of shared memory (the largest tile whose rings fit)
     if (ty == 7) return launch_one<RECON, 7>(p, st);
-    if (ty == 11) return launch_one<RECON, 11>(p, st);
     return cudaErrorInvalidConfiguration;
 }
 
 }  // namespace
 
-bool flux_supported(const RhsParams& p) {
+bool tma_supported(const RhsParams& p) {
     // TMA: global strides are multiples of 16 bytes (even Nx) and the arrays are 16-byte aligned
     if (p.N[0] % 2 != 0) return false;
     if (((uintptr_t)p.prim | (uintptr_t)p.met | (uintptr_t)p.K) & 15u) return false;
     return encode_fn() != nullptr;
 }
 
-cudaError_t launch_rhs_flux(const RhsParams& p, int recon, int ty, cudaStream_t st) {
+cudaError_t launch_rhs_tma(const RhsParams& p, int recon, int ty, cudaStream_t st) {
     if (recon == RECON_WENO5) return dispatch<RECON_WENO5>(p, ty, st);
     if (recon == RECON_MC) return dispatch<RECON_MC>(p, ty, st);
     return dispatch<RECON_MINMOD>(p, ty, st);

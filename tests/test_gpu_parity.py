@@ -29,7 +29,7 @@ def _to_dev(prob):
     return tuple(torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (prob.prim, prob.metric, prob.K))
 
 
-def gpu_rhs(grx, prob, recon, variant="fused", count=False):
+def gpu_rhs(grx, prob, recon, variant="auto", count=False):
     """Runs the CUDA path; `out` is pre-filled with a sentinel so untouched cells are visible."""
     import torch
     prim, met, K = _to_dev(prob)
@@ -44,7 +44,7 @@ def gpu_rhs(grx, prob, recon, variant="fused", count=False):
         torch.cuda.synchronize()
     finally:
         grx.set_fallback_counter(None)
-        grx.set_variant("fused")
+        grx.set_variant("auto")
     res = out.cpu().numpy()
     return (res, int(cnt.item())) if count else res
 
@@ -63,9 +63,11 @@ def check(prob, recon, got, ref, tol=TOL):
 SMALL = ["c1", "gen", "c2:small", "c3:small", "c4:small", "c5-32:small"]
 
 
-@pytest.mark.parametrize("variant", ["fused", "simple", "split", "staged", "ws"])
+@pytest.mark.parametrize("variant", ["auto", "ldg", "simple"])
 @pytest.mark.parametrize("name", SMALL)
 def test_parity_small(grx, oracle, name, variant):
+    """auto = the product path (TMA kernel: every SMALL config has an even Nx), ldg = the round-1 kernel,
+    simple = the one-thread-per-cell cross-check."""
     prob = inputs.by_name(name)
     for recon in prob.recons:
         ref, nfb_ref = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, prob.nghost, recon, prob.gamma)
@@ -74,50 +76,54 @@ def test_parity_small(grx, oracle, name, variant):
         assert nfb == nfb_ref, f"{name}/{recon}: fallback count {nfb} vs oracle {nfb_ref} (R5)"
 
 
-@pytest.mark.parametrize("variant", ["split", "staged", "ws"])
-@pytest.mark.parametrize("n", [(1, 5, 2), (33, 1, 3), (2, 2, 70), (65, 8, 9), (31, 61, 17)])
-def test_parity_variants_ragged(grx, oracle, variant, n):
-    """The split (two barrier-free kernels), staged (cp.async plane in shared memory) and ws (helper warp group
-    for the sources) variants on ragged
-    and thin blocks with an off-diagonal metric: sizes off the 30/32-cell tiles, single rows, long columns."""
-    base = inputs.general_metric_box(n=(66, 62, 71), seed=3, nbox=2)
+@pytest.mark.parametrize("n", [(2, 5, 2), (34, 1, 3), (2, 2, 70), (64, 8, 9), (30, 61, 17), (94, 23, 5), (32, 7, 1),
+                               (66, 15, 40)])
+def test_parity_tma_ragged_and_thin(grx, oracle, n):
+    """The TMA kernel (forced) on ragged and thin blocks with an off-diagonal metric, two boxes: tiles cut by the
+    block edge in x and y (zero-filled part of the TMA box), single rows and columns, blocks smaller than a TMA
+    box, long z chunks, one plane.  All sizes have an even Nx (a TMA requirement)."""
+    base = inputs.general_metric_box(n=(96, 62, 71), seed=3, nbox=2)
     prob = cut_block(base, (1, 1, 1), n)
     for recon in ("minmod", "weno5"):
         ref, nfb_ref = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, prob.nghost, recon, prob.gamma)
-        got, nfb = gpu_rhs(grx, prob, recon, variant, count=True)
+        got, nfb = gpu_rhs(grx, prob, recon, "tma", count=True)
         check(prob, recon, got, ref)
         assert nfb == nfb_ref
 
 
-@pytest.mark.parametrize("variant", ["split", "staged", "ws"])
-def test_parity_variants_two_ghosts_and_rotor(grx, oracle, variant):
-    """minmod/MC with the minimal 2 ghosts (the staged halo must not read outside the array) and the rotor's
-    inadmissible WENO5 face states (R5) through the variants."""
-    prob = inputs.general_metric_box(n=(18, 10, 7), seed=21, g=2)
-    for recon in ("minmod", "mc"):
-        ref, _ = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, 2, recon, prob.gamma)
-        check(prob, recon, gpu_rhs(grx, prob, recon, variant), ref)
+def test_parity_tma_ghost_widths_and_rotor(grx, oracle):
+    """nghost = 2 (minmod/MC; the even-start shift of the TMA boxes differs from nghost = 3), nghost = 4 and 5
+    (wider than needed), and the rotor's inadmissible WENO5 face states (R5) through the TMA kernel."""
+    for g, recons in ((2, ("minmod", "mc")), (4, ("weno5", "mc")), (5, ("weno5", "minmod"))):
+        prob = inputs.general_metric_box(n=(18, 10, 7), seed=21, g=g)
+        for recon in recons:
+            ref, _ = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, g, recon, prob.gamma)
+            check(prob, recon, gpu_rhs(grx, prob, recon, "tma"), ref)
     prob = inputs.rotor((96, 80, 1))
     for recon in prob.recons:
         ref, nfb_ref = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, prob.nghost, recon, prob.gamma)
-        got, nfb = gpu_rhs(grx, prob, recon, variant, count=True)
+        got, nfb = gpu_rhs(grx, prob, recon, "tma", count=True)
         check(prob, recon, got, ref)
         assert nfb == nfb_ref
 
 
-@pytest.mark.parametrize("tile", ["7x2", "11x1", "5x2", "15x1", "7x1", "6x1"])
-def test_parity_all_tiles(grx, oracle, tile, monkeypatch):
-    """Every compiled tile shape of the fused kernel, on a ragged off-diagonal-metric batch and the rotor."""
-    monkeypatch.setenv("GRX_TILE", tile)
-    for prob in (inputs.general_metric_box(n=(37, 19, 11), seed=11, nbox=2), inputs.rotor((96, 80, 1))):
-        for recon in prob.recons:
-            ref, _ = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, prob.nghost, recon, prob.gamma)
-            check(prob, recon, gpu_rhs(grx, prob, recon), ref)
+def test_auto_takes_the_ldg_kernel_for_odd_nx_and_tma_refuses(grx, oracle):
+    """Odd Nx: TMA needs 16-byte global strides, so the product path falls back to the LDG kernel (same bits as
+    forcing it) and forcing TMA is refused with GRX_ERR_UNSUPPORTED before any launch."""
+    prob = inputs.general_metric_box(n=(37, 19, 11), seed=11, nbox=2)
+    for recon in prob.recons:
+        ref, _ = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, prob.nghost, recon, prob.gamma)
+        a = gpu_rhs(grx, prob, recon, "auto")
+        check(prob, recon, a, ref)
+        assert np.array_equal(a[prob.interior], gpu_rhs(grx, prob, recon, "ldg")[prob.interior])
+    with pytest.raises(grx.GrxError, match="error 3"):
+        gpu_rhs(grx, prob, "weno5", "tma")
 
 
 @pytest.mark.parametrize("n", [(1, 1, 1), (1, 5, 2), (33, 1, 3), (2, 2, 70), (65, 8, 9), (31, 23, 17)])
 def test_parity_ragged_and_thin(grx, oracle, n):
-    """Degenerate and ragged block shapes (R24): single cells, thin directions, sizes off the tile grid."""
+    """Degenerate and ragged block shapes (R24) through the product path: single cells, thin directions, sizes off
+    the tile grid (odd sizes take the LDG kernel, even ones the TMA kernel)."""
     base = inputs.general_metric_box(n=(66, 24, 71), seed=3, nbox=2)
     prob = cut_block(base, (1, 1, 1), n)
     for recon in ("minmod", "weno5"):
@@ -192,15 +198,50 @@ def test_parity_config5_128_full(grx, oracle):
         _full_block_check(grx, oracle, prob, recon)
 
 
-def test_fused_equals_simple_variant(grx):
-    """Two independent traversals of the same arithmetic agree to rounding on a batch."""
+def test_three_traversals_agree(grx):
+    """Three traversals of the same arithmetic (TMA kernel, LDG kernel, one thread per cell) agree to rounding on
+    a batch."""
     prob = inputs.general_metric_box(n=(40, 17, 13), seed=5, nbox=3)
     for recon in ("minmod", "mc", "weno5"):
-        a = gpu_rhs(grx, prob, recon, "fused")
+        a = gpu_rhs(grx, prob, recon, "tma")
         ii = prob.interior
-        for other in ("simple", "split", "staged", "ws"):
+        for other in ("simple", "ldg"):
             b = gpu_rhs(grx, prob, recon, other)
             assert relerr_per_component(a[ii], b[ii]).max() < 1e-13, other
+
+
+def test_two_host_threads(grx):
+    """The library keeps no per-launch state: two host threads calling concurrently on their own streams get the
+    bits of a serial call."""
+    import threading
+    import torch
+    prob = inputs.sweep_boxes(32, 2)
+    prim, met, K = _to_dev(prob)
+    serial = grx.valencia_rhs(prim, met, K, prob.dx, prob.nghost, "weno5", prob.gamma)
+    torch.cuda.synchronize()
+    results, errors = [None, None], []
+
+    def work(i):
+        try:
+            torch.cuda.set_device(0)
+            s = torch.cuda.Stream()
+            outs = []
+            for _ in range(5):
+                outs.append(grx.valencia_rhs(prim, met, K, prob.dx, prob.nghost, "weno5", prob.gamma, stream=s))
+            s.synchronize()
+            results[i] = outs
+        except Exception as ex:   # surfaced below
+            errors.append(ex)
+
+    threads = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for outs in results:
+        for o in outs:
+            assert torch.equal(o, serial)
 
 
 def test_batch_equals_single_boxes_bitwise(grx):
