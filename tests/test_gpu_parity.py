@@ -239,9 +239,10 @@ def test_two_host_threads(grx):
     for t in threads:
         t.join()
     assert not errors, errors
+    ii = prob.interior      # ghost cells of `out` are never written (R23): compare the interior
     for outs in results:
         for o in outs:
-            assert torch.equal(o, serial)
+            assert torch.equal(o[ii], serial[ii])
 
 
 def test_batch_equals_single_boxes_bitwise(grx):
