@@ -2,7 +2,7 @@
 """bench.py -- FP64 Valencia RHS cell-updates/s on one 256^3 block (WENO5 + HLLE), B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c5-256]
-                    [--recon weno5|minmod|mc] [--sweep]
+                    [--recon weno5|minmod|mc] [--variant auto|tma|ldg|simple] [--no-sweep] [--sweep]
 
 A "step" is ONE evaluation of the whole hot path (reconstruct -> HLLE -> flux divergence + sources, all three
 directions) over one batch of synthetic input, i.e. one grx_valencia_rhs call = one
@@ -16,7 +16,8 @@ Prints ONE JSON line (rank 0).  `value` = interior cells x boxes x ranks x steps
 HBM; `e2e` = same through grx_valencia_rhs_host with pinned HOST buffers (H2D of all inputs and D2H of the
 result inside the timed region); `roofline` = algorithmic FP64 flops of the launch (the oracle's counted
 operations) / kernel time against the FP64 peak, plus the HBM view; `cpu_baseline` =
-the oracle, as it stands, on the host cores on a bounded sub-block of the same workload.
+the oracle, as it stands, on the host cores on a bounded sub-block of the same workload; `sweep` = every config-5
+point and C3/C4 with both reconstructions (10 calls each), so that the driver-run line carries them.
 
 --impl reference times the oracle (the only reference there is: the paper ships no code) on this host.
 """
@@ -44,11 +45,34 @@ UNIT = "cell-updates/s"
 FLOPS_MODEL = {"weno5": (4753.0, 6210.0), "minmod": (2545.0, 1794.0), "mc": (2642.0, 1460.0)}
 # Nominal FP64 peak of a B200: 148 SMs x 64 FP64 lanes x 2 flop (FMA) x 1.965 GHz.
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE rhs_fused_kernel launch, from the `ncu --set full` capture
-# summarised in profiles/r1_ncu_fused.md (3.968 GB + 1.098 GB); null for workloads that were not captured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {"c5-256/weno5": 5.066e9}
-KERNEL_OF_VARIANT = {"fused": "rhs_fused_kernel", "staged": "rhs_staged_kernel", "simple": "rhs_simple_kernel",
-                     "split": "rhs_z_kernel + rhs_xy_kernel", "ws": "rhs_ws_kernel"}
+# The survey's own estimate of the straightforward formulation: quoted beside the
+# official (oracle-counted) number as `frac_survey_count`.
+FLOPS_SURVEY = {"weno5": 4085.0, "minmod": 2140.0}
+# Numbers that only a profiler can give, from the `ncu --set full` captures summarised under profiles/ (per launch of
+# the kernel of a step): DRAM bytes read + written, FP64-pipe utilisation (% of peak sustained active), executed FP64
+# thread instructions per cell.  They belong to ONE state of the kernel sources: `csrc_sha` is the hash of
+# paper_2210_17509_b200/csrc/ they were captured at, and bench.py reports them only while the hash still matches.
+NCU_CAPTURE = {
+    "csrc_sha": "PENDING",
+    "source": "profiles/r2_ncu_tma.md",
+    "c5-256/weno5/auto": {"traffic": None, "pipe_fp64_pct": None, "fp64_inst_per_cell": None},
+    "c5-256/minmod/auto": {"traffic": None, "pipe_fp64_pct": None, "fp64_inst_per_cell": None},
+}
+KERNEL_OF_VARIANT = {"auto": "rhs_tma_kernel (rhs_fused_kernel for odd Nx)", "tma": "rhs_tma_kernel", "ldg": "rhs_fused_kernel",
+                     "simple": "rhs_simple_kernel"}
+SWEEP_POINTS = ("c5-32", "c5-64", "c5-128", "c5-256", "c3", "c4")
+
+
+def csrc_sha():
+    """Hash of the kernel sources (what NCU_CAPTURE is keyed on)."""
+    import hashlib
+    h = hashlib.sha1()
+    d = os.path.join(ROOT, "paper_2210_17509_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh", ".h")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:12]
 
 
 def algorithmic_flops_per_cell(n, recon):
@@ -357,13 +381,27 @@ def run_ours(args):
         "unit": "TFLOP/s", "frac": ach_tflops / FP64_PEAK_NOMINAL_TFLOPS,
         "peak_source": "nominal FP64: 148 SM x 64 lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry)",
         "peak_dfma_measured": dfma, "frac_of_dfma_measured": ach_tflops / dfma if dfma > 0 else None,
-        "flops_per_cell": fl_cell, "bytes_per_cell": by_cell,
+        "flops_per_cell": fl_cell, "flops_source": "operations of the oracle's counting instance, pinned piece by piece "
+                                                   "against hand counts (tests/test_bench_model.py)",
+        "frac_survey_count": (FLOPS_SURVEY[recon] * cells / t_launch / 1e12 / FP64_PEAK_NOMINAL_TFLOPS
+                              if recon in FLOPS_SURVEY else None),
+        "flops_per_cell_survey": FLOPS_SURVEY.get(recon),
+        "bytes_per_cell": by_cell,
         "hbm": {"achieved": ach_gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s", "peak_source": peak_src,
                 "frac": ach_gbs / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None},
         "traffic": None,
     }
-    if args.variant == "fused":
-        roofline["traffic"] = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(f"{args.workload}/{recon}")
+    # profiler-only numbers: reported only for the state of the kernel sources they were captured at
+    sha = csrc_sha()
+    cap = NCU_CAPTURE.get(f"{args.workload}/{recon}/{args.variant}")
+    if cap and NCU_CAPTURE["csrc_sha"] == sha:
+        roofline["traffic"] = cap["traffic"]
+        roofline["ncu"] = dict(cap, source=NCU_CAPTURE["source"], csrc_sha=sha)
+        if cap.get("fp64_inst_per_cell"):
+            # one executed FP64 instruction = one lane-slot of the pipe whatever it does (an FMA counts 2 flops)
+            roofline["frac_executed_slots"] = cap["fp64_inst_per_cell"] * cells / t_launch / (148 * 64 * 1.965e9)
+    else:
+        roofline["ncu"] = {"csrc_sha": sha, "note": "no ncu capture for this state of csrc/ (captured at %s)" % NCU_CAPTURE["csrc_sha"]}
 
     # ---- the oracle on the host cores, bounded sample of the same workload
     cpu_rate, cpu_t, n1, cores = time_oracle(prob, recon, budget_s=args.cpu_seconds)
@@ -371,26 +409,61 @@ def run_ours(args):
                     "sample": f"first {n1[0]}x{n1[1]}x{n1[2]} interior cells (+3 ghosts) of the same block, "
                               f"one evaluation, {cpu_t:.1f} s"}
 
+    sweep = None
+    if not args.no_sweep and args.workload == "c5-256":
+        sweep = sweep_points(grx, torch, stream, SWEEP_POINTS, 10, 3, peaks, keep=("c5-256", prob, dev))
+
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"{prob.name} per GPU, {recon}+HLLE, Gamma-law EOS, perturbed conformally flat metric "
                                f"+ shift + K_ij, {g} ghosts; one grx_valencia_rhs call per step",
-                   "l2": "inputs 4.6 GB >> 126 MB L2, no flush", "tile": os.environ.get("GRX_TILE", "default"), "variant": args.variant,
+                   "l2": "inputs 4.6 GB >> 126 MB L2, no flush", "variant": args.variant,
                    "parallelism": f"blocks x{world}, no collective"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "matches_device_path": e2e_ok},
-        "gpu_launches": args.steps * (2 if args.variant == "split" else 1),
+        "gpu_launches": args.steps,
         "roofline": roofline,
         "cpu_baseline": cpu_baseline,
     }
+    if sweep is not None:
+        line["sweep"] = sweep
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
     return 0
+
+
+def sweep_points(grx, torch, stream, names, steps, warmup, peaks, keep=None):
+    """Times every (workload, reconstruction) point: `steps` calls after `warmup`, CUDA events on the launching
+    stream.  One workload is resident at a time (inputs are generated per point to bound host memory).  `keep` is an
+    already loaded (name, prob, dev) that is reused instead of being generated again."""
+    pts = []
+    for name in names:
+        if keep is not None and keep[0] == name:
+            prob, dev, own = keep[1], keep[2], False
+        else:
+            prob = load_workload(name, 0)
+            dev = tuple(torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (prob.prim, prob.metric, prob.K))
+            own = True
+        for recon in prob.recons:
+            t, _ = time_rhs(grx, torch, prob, dev, recon, steps, max(warmup, 3), stream)
+            tl = t / steps
+            fl = algorithmic_flops_per_cell(prob.n, recon) * prob.cells / tl / 1e12
+            gb = algorithmic_bytes_per_cell(prob.n, prob.nghost) * prob.cells / tl / 1e9
+            pt = {"workload": prob.name, "recon": recon, "cells": prob.cells, "ms_per_call": 1e3 * tl,
+                  "cell_updates_per_s": prob.cells / tl, "frac": fl / FP64_PEAK_NOMINAL_TFLOPS,
+                  "hbm_frac": gb / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None}
+            if recon in FLOPS_SURVEY:
+                pt["frac_survey_count"] = FLOPS_SURVEY[recon] * prob.cells / tl / 1e12 / FP64_PEAK_NOMINAL_TFLOPS
+            pts.append(pt)
+        if own:
+            del dev, prob
+            torch.cuda.empty_cache()
+    return pts
 
 
 def run_sweep(args):
@@ -401,20 +474,9 @@ def run_sweep(args):
     grx.lib()
     grx.set_variant(args.variant)
     stream = torch.cuda.current_stream()
-    for name in ("c5-32", "c5-64", "c5-128", "c5-256", "c4", "c3", "c2", "c1"):
-        prob = load_workload(name, 0)
-        dev = tuple(torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (prob.prim, prob.metric, prob.K))
-        for recon in prob.recons:
-            t, _ = time_rhs(grx, torch, prob, dev, recon, args.steps, max(args.warmup, 3), stream)
-            tl = t / args.steps
-            fl = algorithmic_flops_per_cell(prob.n, recon) * prob.cells / tl / 1e12
-            gb = algorithmic_bytes_per_cell(prob.n, prob.nghost) * prob.cells / tl / 1e9
-            print(json.dumps({"workload": prob.name, "recon": recon, "cells": prob.cells, "us_per_call": 1e6 * tl,
-                              "cell_updates_per_s": prob.cells / tl, "tflops_alg": fl,
-                              "frac_fp64_nominal": fl / FP64_PEAK_NOMINAL_TFLOPS, "gbs_alg": gb,
-                              "tile": os.environ.get("GRX_TILE", "default")}), flush=True)
-        del dev
-        torch.cuda.empty_cache()
+    peaks, _ = measured_peaks()
+    for pt in sweep_points(grx, torch, stream, SWEEP_POINTS + ("c2", "c1"), args.steps, args.warmup, peaks):
+        print(json.dumps(pt), flush=True)
     return 0
 
 
@@ -427,8 +489,9 @@ def main():
     ap.add_argument("--workload", default="c5-256")
     ap.add_argument("--recon", default="weno5", choices=["weno5", "minmod", "mc"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="wall-clock budget of the oracle sample")
-    ap.add_argument("--variant", default="fused", choices=["fused", "staged", "split", "ws", "simple"],
-                    help="kernel variant (fused = product path)")
+    ap.add_argument("--variant", default="auto", choices=["auto", "tma", "ldg", "simple"],
+                    help="kernel selector (auto = product path)")
+    ap.add_argument("--no-sweep", action="store_true", help="leave the config sweep out of the contract line")
     ap.add_argument("--sweep", action="store_true", help="time every config instead of the contract line")
     args = ap.parse_args()
     if args.steps < 1:

@@ -58,7 +58,21 @@ cudaError_t launch_variant(const grx::RhsParams& p, int recon, cudaStream_t st, 
         if (unsupported) *unsupported = true;
         return cudaErrorNotSupported;
     }
-    return ok ? grx::launch_rhs_tma(p, recon, 7, st) : grx::launch_rhs_fused(p, recon, st);
+    if (!ok) return grx::launch_rhs_fused(p, recon, st);
+    if (variant == GRX_VARIANT_AUTO) {
+        // Both kernels take the block: choose by the expected time.  Per cell of a well-filled machine the TMA kernel
+        // is about 1.12x (WENO5) to 1.22x (TVD) faster; on small blocks and batches its 7-row tiles and its per-chunk
+        // set-up fill the SMs less well than the LDG kernel's 11-row tiles (constants fitted on the config-5 sweep,
+        // profiles/r2_sweep.md: the selector picks the faster kernel at every point).
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) {
+            const double gain = (recon == GRX_RECON_WENO5) ? 1.12 : 1.22;
+            if (gain * grx::tma_tile_efficiency(p, sms) < grx::fused_tile_efficiency(p, sms))
+                return grx::launch_rhs_fused(p, recon, st);
+        }
+    }
+    return grx::launch_rhs_tma(p, recon, 7, st);
 }
 
 // The two internal streams of grx_valencia_rhs_host: one pair per host thread and device, created on first use.

@@ -267,7 +267,7 @@ namespace {
 
 // z-chunking: enough CTAs to fill the machine a few times over, chunks long enough to amortise the two
 // one-sided plane steps at their ends.
-TileGeom make_tiles(const RhsParams& p, int ty, int slots) {
+TileGeom make_tiles(const RhsParams& p, int ty, int slots, double* eff_out = nullptr) {
     TileGeom tg;
     tg.ntx = (p.n[0] + TX - 1) / TX;
     tg.nty = (p.n[1] + ty - 1) / ty;
@@ -287,6 +287,7 @@ TileGeom make_tiles(const RhsParams& p, int ty, int slots) {
     tg.tz = (p.n[2] + best - 1) / best;
     tg.nzc = (p.n[2] + tg.tz - 1) / tg.tz;
     tg.pf = 3;   // software prefetch of the first-touch lines (profiles/r1_variants.md)
+    if (eff_out) *eff_out = best_eff * p.n[1] / ((double)tg.nty * ty);
     return tg;
 }
 
@@ -317,6 +318,12 @@ cudaError_t dispatch(const RhsParams& p, cudaStream_t st) {
 }
 
 }  // namespace
+
+double fused_tile_efficiency(const RhsParams& p, int sms) {
+    double eff = 0.0;
+    make_tiles(p, p.n[2] < 8 ? 7 : 11, sms, &eff);
+    return eff;
+}
 
 cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st) {
     if (recon == RECON_WENO5) return dispatch<RECON_WENO5>(p, st);

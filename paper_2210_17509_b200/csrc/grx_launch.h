@@ -11,10 +11,12 @@ namespace grx {
 cudaError_t launch_rhs_simple(const RhsParams& p, int recon, cudaStream_t st);
 // grx_fused.cu: the round-1 kernel (operands through L1), the path for arrays the TMA kernel cannot take
 cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st);
+double fused_tile_efficiency(const RhsParams& p, int sms);   // expected fill of the launch geometry, in (0, 1]
 
 // grx_tma.cu: the product kernel (TMA-staged planes, shared-memory z rings); needs even Nx and 16-byte aligned arrays
 bool tma_supported(const RhsParams& p);
 cudaError_t launch_rhs_tma(const RhsParams& p, int recon, int ty, cudaStream_t st);
+double tma_tile_efficiency(const RhsParams& p, int sms);
 
 // grx_support.cu
 cudaError_t launch_prim2con(const double* prim, const double* met, long long nc, int nbox, double gamma, double* cons,

@@ -511,9 +511,12 @@ bool make_map(CUtensorMap* map, const double* base, const RhsParams& p, int nf, 
     return r == CUDA_SUCCESS;
 }
 
-// z-chunking: enough CTAs to fill the machine in whole waves, chunks long enough to amortise the two one-sided
-// plane steps at their ends.
-TmaGeom make_tiles(const RhsParams& p, int ty, int slots) {
+// z-chunking: enough CTAs to fill the machine in whole waves, chunks long enough to amortise what a chunk costs
+// besides its planes: the ring fill, the first TMA round trip and the two one-sided plane steps at its ends
+// (together about 1.8 plane steps, measured on the 32^3 and 64^3 batches).  Returns the expected efficiency
+// (wave fill x chunk factor x used rows of the row tiles) in *eff.
+constexpr double CHUNK_OVERHEAD = 1.8;
+TmaGeom make_tiles(const RhsParams& p, int ty, int slots, double* eff_out = nullptr) {
     TmaGeom tg;
     tg.ntx = (p.n[0] + TX - 1) / TX;
     tg.nty = (p.n[1] + ty - 1) / ty;
@@ -527,11 +530,12 @@ TmaGeom make_tiles(const RhsParams& p, int ty, int slots) {
         if (real != nzc) continue;
         const double waves = (double)(inplane * nzc) / slots;
         const double fill = waves / (double)(long long)(waves + 0.999999);
-        const double eff = fill * tz / (tz + 0.45);
+        const double eff = fill * tz / (tz + CHUNK_OVERHEAD);
         if (eff > best_eff * 1.001) { best_eff = eff; best = nzc; }
     }
     tg.tz = (p.n[2] + best - 1) / best;
     tg.nzc = (p.n[2] + tg.tz - 1) / tg.tz;
+    if (eff_out) *eff_out = best_eff * p.n[1] / ((double)tg.nty * ty);
     return tg;
 }
 
@@ -571,6 +575,12 @@ bool tma_supported(const RhsParams& p) {
     if (p.N[0] % 2 != 0) return false;
     if (((uintptr_t)p.prim | (uintptr_t)p.met | (uintptr_t)p.K) & 15u) return false;
     return encode_fn() != nullptr;
+}
+
+double tma_tile_efficiency(const RhsParams& p, int sms) {
+    double eff = 0.0;
+    make_tiles(p, 7, sms, &eff);
+    return eff;
 }
 
 cudaError_t launch_rhs_tma(const RhsParams& p, int recon, int ty, cudaStream_t st) {
