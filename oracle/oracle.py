@@ -35,6 +35,9 @@ def lib():
         L.oracle_prim2con.restype = C.c_int
         L.oracle_con2prim.argtypes = [ip, C.c_int, dp, dp, C.c_int, C.c_double, dp]
         L.oracle_con2prim.restype = C.c_int
+        L.oracle_evolve.argtypes = [ip, C.c_int, dp, dp, dp, dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int,
+                                    C.c_int, dp]
+        L.oracle_evolve.restype = C.c_int
         L.oracle_recon_cell.argtypes = [C.c_int, dp, dp, dp]
         L.oracle_recon_cell.restype = None
         L.oracle_state_flux.argtypes = [dp, dp, C.c_int, C.c_double, dp, dp, dp]
@@ -112,6 +115,25 @@ def con2prim(cons, metric, nghost, gamma):
     if nfail < 0:
         raise ValueError("oracle: invalid argument")
     return prim, nfail
+
+
+BC = {"copy": 0, "periodic": 1}
+
+
+def evolve(prim, metric, K, dx, nghost, recon, gamma, dt, nsteps, rk=2, bc="copy"):
+    """Method of lines around the right-hand side (oracle_evolve): returns (prim, cons, nfail) after `nsteps` steps;
+    `prim` must come with filled ghosts and is not modified."""
+    prim = np.array(prim, dtype=np.float64, order="C", copy=True)
+    metric, K = _arr(metric), _arr(K)
+    n, nbox = _grid(prim, nghost)
+    cons = np.zeros_like(prim)
+    dxa = (C.c_double * 3)(*dx)
+    r = RECON[recon] if isinstance(recon, str) else int(recon)
+    nfail = lib().oracle_evolve(n, nbox, _p(prim), _p(metric), _p(K), dxa, nghost, r, gamma, dt, int(nsteps), int(rk),
+                                BC[bc], _p(cons))
+    if nfail < 0:
+        raise ValueError("oracle: invalid argument")
+    return prim, cons, nfail
 
 
 def recon_cell(recon, q5):

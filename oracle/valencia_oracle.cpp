@@ -486,8 +486,19 @@ int rhs_all(const int n[3], int nbox, const double* prim, const double* met, con
     return 0;
 }
 
-// ---- support code for the short Balsara-1 evolution (R21, R22): ideal-gas con2prim -----------------------
-// 1-D Newton/bisection solve in z = rho h W^2 on the undensitised conserved variables.
+// ---- NEXT-1: ideal-gas con2prim and the method-of-lines loop ----------------------------
+// con2prim (PAPER.md l.129 step 1, l.142-146; reading R22): 1-D solve in z = rho h W^2 on the undensitised
+// conserved variables,
+//   v^2(z) = [S^2 z^2 + (S.B)^2 (B^2 + 2 z)] / [(z + B^2)^2 z^2],   W = (1 - v^2)^(-1/2),   rho = D / W,
+//   p(z) = (Gamma-1)/Gamma (z / W^2 - rho),
+//   f(z) = z + B^2 - p - B^2 / (2 W^2) - (S.B)^2 / (2 z^2) - (tau + D) = 0,
+// by Newton's method with the ANALYTIC derivative
+//   (v^2)' = (N' Dn - N Dn') / Dn^2,  N = S^2 z^2 + (S.B)^2 (B^2 + 2z),  Dn = (z + B^2)^2 z^2,
+//   p' = (Gamma-1)/Gamma [ (1 - v^2) - z (v^2)' + D (v^2)' / (2 sqrt(1 - v^2)) ],
+//   f' = 1 - p' + (B^2/2) (v^2)' + (S.B)^2 / z^3,
+// safeguarded by a bracket [zlo, zhi] with f(zlo) < 0 < f(zhi) (bisection step whenever Newton leaves it), stopped at
+// |dz| < 1e-14 z.  (The CUDA path solves the same equation with a finite-difference slope; the two share the equation,
+// not the iteration.)
 int con2prim_point(const double U[8], const Metric<double>& m, double gamma, double P[8]) {
     const double sg = m.sqrtg;
     const double D = U[0] / sg, tau = U[4] / sg;
@@ -501,40 +512,60 @@ int con2prim_point(const double U[8], const Metric<double>& m, double gamma, dou
     const double S2 = Sl[0] * Su[0] + Sl[1] * Su[1] + Sl[2] * Su[2];
     const double B2 = Bl[0] * B[0] + Bl[1] * B[1] + Bl[2] * B[2];
     const double SB = Sl[0] * B[0] + Sl[1] * B[1] + Sl[2] * B[2];
-    const double E = tau + D;
-    auto eval = [&](double z, double& W, double& rho, double& p) {
-        double v2 = (S2 * z * z + SB * SB * (B2 + 2.0 * z)) / ((z + B2) * (z + B2) * z * z);
-        if (v2 > 1.0 - 1e-15) v2 = 1.0 - 1e-15;
-        W = 1.0 / std::sqrt(1.0 - v2);
-        rho = D / W;
-        p = (gamma - 1.0) / gamma * (z / (W * W) - rho);
-        return z + B2 - p - B2 / (2.0 * W * W) - SB * SB / (2.0 * z * z) - E;
+    const double T = SB * SB, E = tau + D, cg = (gamma - 1.0) / gamma;
+    // f and f' at z
+    auto eval = [&](double z, double& fp) {
+        const double N = S2 * z * z + T * (B2 + 2.0 * z);
+        const double zb = z + B2, Dn = zb * zb * z * z;
+        const double dN = 2.0 * S2 * z + 2.0 * T, dDn = 2.0 * z * zb * (2.0 * z + B2);
+        double x = N / Dn, dx = (dN * Dn - N * dDn) / (Dn * Dn);
+        if (x > 1.0 - 1e-15) { x = 1.0 - 1e-15; dx = 0.0; }
+        const double w = std::sqrt(1.0 - x);            // 1/W
+        const double p = cg * (z * (1.0 - x) - D * w);
+        const double dp = cg * ((1.0 - x) - z * dx + D * dx / (2.0 * w));
+        fp = 1.0 - dp + 0.5 * B2 * dx + T / (z * z * z);
+        return z + B2 - p - 0.5 * B2 * (1.0 - x) - T / (2.0 * z * z) - E;
     };
-    // bracket: f is increasing in z for physical states
-    double W, rho, p;
-    double zlo = 1e-300, zhi = std::fmax(2.0 * (E + 1.0), 1.0);
-    for (int it = 0; it < 200 && eval(zhi, W, rho, p) < 0.0; ++it) zhi *= 2.0;
-    zlo = zhi;
-    for (int it = 0; it < 400 && eval(zlo, W, rho, p) > 0.0; ++it) zlo *= 0.5;
+    double fp;
+    double zhi = std::fmax(2.0 * (E + 1.0), 1.0);
+    for (int it = 0; it < 200 && eval(zhi, fp) < 0.0; ++it) zhi *= 2.0;
+    double zlo = zhi;
+    for (int it = 0; it < 400 && eval(zlo, fp) > 0.0; ++it) zlo *= 0.5;
     double z = 0.5 * (zlo + zhi);
     int status = 1;
     for (int it = 0; it < 200; ++it) {
-        double f = eval(z, W, rho, p);
+        const double f = eval(z, fp);
         if (f > 0.0) zhi = z; else zlo = z;
-        const double h = 1e-6 * z;
-        double fp = (eval(z + h, W, rho, p) - eval(z - h, W, rho, p)) / (2.0 * h);
         double zn = z - f / fp;
         if (!(zn > zlo && zn < zhi)) zn = 0.5 * (zlo + zhi);
         const double dz = std::fabs(zn - z);
         z = zn;
         if (dz < 1e-14 * z) { status = 0; break; }
     }
-    eval(z, W, rho, p);
+    const double N = S2 * z * z + T * (B2 + 2.0 * z), zb = z + B2;
+    double x = N / (zb * zb * z * z);
+    if (x > 1.0 - 1e-15) x = 1.0 - 1e-15;
+    const double w = std::sqrt(1.0 - x);
+    const double rho = D * w, p = cg * (z * (1.0 - x) - rho);
     P[0] = rho;
-    for (int i = 0; i < 3; ++i) P[1 + i] = (Su[i] + SB * B[i] / z) / (z + B2);
+    for (int i = 0; i < 3; ++i) P[1 + i] = (Su[i] + SB * B[i] / z) / zb;
     P[4] = p / ((gamma - 1.0) * rho);
     for (int i = 0; i < 3; ++i) P[5 + i] = B[i];
     return status;
+}
+
+// Ghost fill of the 8 primitive fields of one box at the outer boundary (l.170, l.255, l.329): bc = 0 "copy" (von
+// Neumann: the nearest interior cell), bc = 1 periodic.  Every ghost cell takes the interior cell whose index is the
+// clamped / wrapped ghost index, direction by direction.
+void fill_ghosts_box(const Grid& G, double* prim, int bc) {
+    auto src = [&](int i, int n) { return bc == 1 ? ((i % n) + n) % n : (i < 0 ? 0 : (i >= n ? n - 1 : i)); };
+    for (int q = 0; q < 8; ++q)
+        for (int k = -G.g; k < G.n[2] + G.g; ++k)
+            for (int j = -G.g; j < G.n[1] + G.g; ++j)
+                for (int i = -G.g; i < G.n[0] + G.g; ++i) {
+                    const int si = src(i, G.n[0]), sj = src(j, G.n[1]), sk = src(k, G.n[2]);
+                    if (si != i || sj != j || sk != k) prim[q * G.ncell + G.idx(i, j, k)] = prim[q * G.ncell + G.idx(si, sj, sk)];
+                }
 }
 
 }  // namespace
@@ -617,6 +648,95 @@ int oracle_con2prim(const int n[3], int nbox, const double* cons, const double* 
             for (int q = 0; q < 8; ++q) pb[q * NC + c0] = P[q];
         }
     }
+    return nfail;
+}
+
+// NEXT-1: method of lines (l.125) around the right-hand side, `nsteps` steps of size dt on every box.
+//   rk = 2: SSP-RK2 (Heun; reading R21)   U1 = U + dt L(P);  U <- 1/2 U + 1/2 (U1 + dt L(P1))
+//   rk = 4: classical RK4 (l.255, l.335)   U <- U + dt/6 (k1 + 2 k2 + 2 k3 + k4),  k2 = L(P(U + dt/2 k1)), ...
+// The evolved variables are the conserved ones on the interior cells; after every stage update the primitives follow by
+// con2prim on the interior (step 1 of the paper's RHS evaluation, l.129) and their ghost zones are filled (bc = 0 copy,
+// 1 periodic).  prim (in/out) must come with filled ghosts; cons (out, may be NULL) receives U on the interior (ghosts 0).
+// Returns the number of con2prim failures (>= 0) or -1 for invalid arguments.
+int oracle_evolve(const int n[3], int nbox, double* prim, const double* metric, const double* K, const double dx[3],
+                  int nghost, int recon, double gamma, double dt, int nsteps, int rk, int bc, double* cons) {
+    if (!n || !prim || !metric || !K || !dx || nbox < 1 || nsteps < 0 || (rk != 2 && rk != 4) || (bc != 0 && bc != 1)) return -1;
+    if (!(gamma > 1.0) || nghost < (recon == RECON_WENO5 ? 3 : 2)) return -1;
+    Grid G;
+    G.g = nghost;
+    G.ncell = 1;
+    for (int a = 0; a < 3; ++a) { G.n[a] = n[a]; G.N[a] = n[a] + 2 * nghost; G.ncell *= (size_t)G.N[a]; }
+    const size_t NC = G.ncell, NA = 8 * NC * (size_t)nbox;
+    std::vector<double> U(NA, 0.0), U0(NA), L(NA), acc;
+    if (oracle_prim2con(n, nbox, prim, metric, nghost, gamma, U.data())) return -1;
+    int nfail = 0;
+    // U_out = a U0 + b (U_in + dt L) on the interior, then prim = con2prim(U_out) there and ghost fill
+    auto stage = [&](double a, const std::vector<double>& Ua, double b, const std::vector<double>& Ub, double h,
+                     std::vector<double>& Uout) {
+        for (int bx = 0; bx < nbox; ++bx) {
+            const size_t off = (size_t)bx * 8 * NC;
+            const double* mb = metric + (size_t)bx * 10 * NC;
+            int nf = 0;
+#pragma omp parallel for schedule(static) collapse(2) reduction(+ : nf)
+            for (int k = 0; k < G.n[2]; ++k)
+                for (int j = 0; j < G.n[1]; ++j)
+                    for (int i = 0; i < G.n[0]; ++i) {
+                        const size_t c0 = G.idx(i, j, k);
+                        double Uc[8], P[8];
+                        for (int q = 0; q < 8; ++q) {
+                            const size_t o = off + q * NC + c0;
+                            Uc[q] = a * Ua[o] + b * (Ub[o] + h * L[o]);
+                            Uout[o] = Uc[q];
+                        }
+                        Metric<double> m;
+                        m.alp = mb[c0];
+                        for (int d = 0; d < 3; ++d) m.beta[d] = mb[(1 + d) * NC + c0];
+                        for (int c = 0; c < 6; ++c) m.g[c] = mb[(4 + c) * NC + c0];
+                        metric_complete(m);
+                        nf += con2prim_point(Uc, m, gamma, P);
+                        for (int q = 0; q < 8; ++q) prim[off + q * NC + c0] = P[q];
+                    }
+            nfail += nf;
+            fill_ghosts_box(G, prim + off, bc);
+        }
+    };
+    auto rhs = [&]() { return rhs_all<double>(n, nbox, prim, metric, K, dx, nghost, recon, gamma, L.data(), nullptr, nullptr); };
+    for (int s = 0; s < nsteps; ++s) {
+        U0 = U;
+        if (rk == 2) {
+            if (rhs()) return -1;
+            stage(0.0, U0, 1.0, U0, dt, U);          // U1 = U0 + dt L(P0)
+            if (rhs()) return -1;
+            stage(0.5, U0, 0.5, U, dt, U);           // U  = 1/2 U0 + 1/2 (U1 + dt L(P1))
+        } else {
+            acc = U0;                                 // acc = U0 + dt/6 (k1 + 2 k2 + 2 k3 + k4), built stage by stage
+            const double w[4] = {1.0 / 6.0, 1.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0}, hs[3] = {0.5, 0.5, 1.0};
+            for (int st = 0; st < 4; ++st) {
+                if (rhs()) return -1;
+                for (int bx = 0; bx < nbox; ++bx)
+                    for (int q = 0; q < 8; ++q)
+                        for (int k = 0; k < G.n[2]; ++k)
+                            for (int j = 0; j < G.n[1]; ++j)
+                                for (int i = 0; i < G.n[0]; ++i) {
+                                    const size_t o = (size_t)bx * 8 * NC + q * NC + G.idx(i, j, k);
+                                    acc[o] += w[st] * dt * L[o];
+                                }
+                if (st < 3) stage(0.0, U0, 1.0, U0, hs[st] * dt, U);   // U = U0 + h dt k_st
+                else { for (size_t o = 0; o < NA; ++o) L[o] = 0.0; stage(0.0, U0, 1.0, acc, 0.0, U); }
+            }
+        }
+    }
+    if (cons)
+        for (size_t o = 0; o < NA; ++o) cons[o] = 0.0;
+    if (cons)
+        for (int bx = 0; bx < nbox; ++bx)
+            for (int q = 0; q < 8; ++q)
+                for (int k = 0; k < G.n[2]; ++k)
+                    for (int j = 0; j < G.n[1]; ++j)
+                        for (int i = 0; i < G.n[0]; ++i) {
+                            const size_t o = (size_t)bx * 8 * NC + q * NC + G.idx(i, j, k);
+                            cons[o] = U[o];
+                        }
     return nfail;
 }
 
