@@ -121,6 +121,28 @@ int grx_con2prim(const grx_grid* grid, const double* cons, const double* metric,
 int grx_rk_axpy(const grx_grid* grid, int nghost, double a, const double* x, double b, double dt,
                 const double* rhs, double* y, void* cuda_stream);
 
+/* NEXT-1: `nsteps` time steps of the method of lines around the right-hand
+ * side, entirely on the device and on the caller's stream -- no host round trip between stages.  Every stage is
+ *   L = grx_valencia_rhs(prim);   U <- a U0 + b (U + h L) on the interior, FUSED with con2prim of the new U (step 1 of the
+ *   paper's RHS evaluation, l.129; Gamma-law, R22) and, for RK4, with the accumulation of U0 + dt/6 (k1 + 2k2 + 2k3 + k4);
+ *   ghost fill of the 8 primitives at the outer boundary (l.170): GRX_BC_COPY (von Neumann "copy", l.255) or
+ *   GRX_BC_PERIODIC (l.329).
+ * rk_order 2 = SSP-RK2 / Heun (R21), 4 = classical RK4 (l.255, l.335).
+ *   cons    [nbox][8][Nz][Ny][Nx]  in/out: conserved variables on the INTERIOR cells (e.g. from grx_prim2con); ghosts unused.
+ *   prim    [nbox][8][Nz][Ny][Nx]  in/out: primitives with FILLED ghosts, consistent with cons; on return those of the new
+ *           time level, ghosts filled.
+ *   metric, K, dx, nghost, recon, gamma: as for grx_valencia_rhs (static spacetime: they are not evolved).
+ *   workspace  DEVICE pointer, at least grx_step_workspace_bytes(grid, nghost, rk_order) bytes (2 arrays of the size of
+ *           cons for RK2, 3 for RK4), owned by the caller.
+ *   nfail   DEVICE pointer to one unsigned long long (caller-zeroed) or NULL: incremented by the number of cells whose
+ *           con2prim did not converge.
+ * Returns GRX_OK, GRX_ERR_INVALID_ARG or GRX_ERR_CUDA. */
+enum { GRX_BC_COPY = 0, GRX_BC_PERIODIC = 1 };
+size_t grx_step_workspace_bytes(const grx_grid* grid, int nghost, int rk_order);
+int grx_step_rk(const grx_grid* grid, double* cons, double* prim, const double* metric, const double* K,
+                const double dx[3], int nghost, int recon, double gamma, double dt, int rk_order, int bc, int nsteps,
+                void* workspace, size_t workspace_bytes, unsigned long long* nfail, void* cuda_stream);
+
 /* Debug: if `counter` (DEVICE pointer to one unsigned long long, caller-zeroed) is non-NULL, later
  * grx_valencia_rhs calls of this host thread add to it the number of face sides that took the R5
  * first-order fallback.  NULL switches counting off (the default; counting costs a few atomics). */

@@ -285,6 +285,72 @@ int grx_rk_axpy(const grx_grid* grid, int nghost, double a, const double* x, dou
     return GRX_OK;
 }
 
+size_t grx_step_workspace_bytes(const grx_grid* grid, int nghost, int rk_order) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (make_geom(grid, nghost, p) || (rk_order != 2 && rk_order != 4)) return 0;
+    return (size_t)(rk_order == 2 ? 2 : 3) * 8 * (size_t)p.nc * (size_t)p.nbox * sizeof(double);
+}
+
+int grx_step_rk(const grx_grid* grid, double* cons, double* prim, const double* metric, const double* K,
+                const double dx[3], int nghost, int recon, double gamma, double dt, int rk_order, int bc, int nsteps,
+                void* workspace, size_t workspace_bytes, unsigned long long* nfail, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!cons || !prim || !metric || !K || !dx || !workspace) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (recon != GRX_RECON_MINMOD && recon != GRX_RECON_MC && recon != GRX_RECON_WENO5)
+        return fail(GRX_ERR_INVALID_ARG, "unknown recon");
+    if (nghost < (recon == GRX_RECON_WENO5 ? 3 : 2))
+        return fail(GRX_ERR_INVALID_ARG, "nghost too small: WENO5 needs 3, minmod/MC need 2 (R29)");
+    if (!(gamma > 1.0)) return fail(GRX_ERR_INVALID_ARG, "gamma must be > 1");
+    if (rk_order != 2 && rk_order != 4) return fail(GRX_ERR_INVALID_ARG, "rk_order must be 2 or 4");
+    if (bc != GRX_BC_COPY && bc != GRX_BC_PERIODIC) return fail(GRX_ERR_INVALID_ARG, "unknown boundary condition");
+    if (nsteps < 0 || !(dt == dt)) return fail(GRX_ERR_INVALID_ARG, "nsteps must be >= 0 and dt a number");
+    for (int a = 0; a < 3; ++a) {
+        if (!(dx[a] > 0.0) || !(1.0 / dx[a] > 0.0)) return fail(GRX_ERR_INVALID_ARG, "dx must be > 0 and finite");
+        p.idx[a] = 1.0 / dx[a];
+    }
+    const size_t arr = 8 * (size_t)p.nc * (size_t)p.nbox;
+    if (workspace_bytes < (size_t)(rk_order == 2 ? 2 : 3) * arr * sizeof(double))
+        return fail(GRX_ERR_INVALID_ARG, "workspace too small");
+    double* U0 = static_cast<double*>(workspace);
+    double* L = U0 + arr;
+    double* acc = rk_order == 4 ? L + arr : nullptr;
+    p.prim = prim; p.met = metric; p.K = K; p.out = L;
+    p.gamma = gamma;
+    p.nfallback = nullptr;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    cudaError_t e = cudaSuccess;
+    auto rhs = [&]() { return launch_variant(p, recon, st); };
+    auto stage = [&](double a, const double* Ua, double b, const double* Ub, double h, double* ac, double wdt) {
+        cudaError_t r = grx::launch_rk_stage(p, a, Ua, b, Ub, h, L, cons, ac, wdt, prim, nfail, st);
+        return r != cudaSuccess ? r : grx::launch_fill_ghosts(p, prim, bc, st);
+    };
+    // L lives in the workspace: its ghost cells are never read or written
+    for (int s = 0; s < nsteps && e == cudaSuccess; ++s) {
+        e = cudaMemcpyAsync(U0, cons, arr * sizeof(double), cudaMemcpyDeviceToDevice, st);
+        if (rk_order == 2) {
+            if (e == cudaSuccess) e = rhs();
+            if (e == cudaSuccess) e = stage(0.0, U0, 1.0, U0, dt, nullptr, 0.0);       // U1 = U0 + dt L(P0)
+            if (e == cudaSuccess) e = rhs();
+            if (e == cudaSuccess) e = stage(0.5, U0, 0.5, cons, dt, nullptr, 0.0);     // U = 1/2 U0 + 1/2 (U1 + dt L(P1))
+        } else {
+            const double w[4] = {1.0 / 6.0, 1.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0}, hs[3] = {0.5, 0.5, 1.0};
+            if (e == cudaSuccess) e = cudaMemcpyAsync(acc, cons, arr * sizeof(double), cudaMemcpyDeviceToDevice, st);
+            for (int k = 0; k < 3 && e == cudaSuccess; ++k) {
+                e = rhs();
+                if (e == cudaSuccess) e = stage(0.0, U0, 1.0, U0, hs[k] * dt, acc, w[k] * dt);   // U = U0 + h dt k_k
+            }
+            if (e == cudaSuccess) e = rhs();
+            // the last weight goes in as the stage's own step: U = (U0 + dt/6 (k1 + 2 k2 + 2 k3)) + dt/6 k4
+            if (e == cudaSuccess) e = stage(0.0, U0, 1.0, acc, w[3] * dt, nullptr, 0.0);         // U = acc + dt/6 k4
+        }
+    }
+    if (e != cudaSuccess) return fail_cuda(e, "grx_step_rk");
+    return GRX_OK;
+}
+
 int grx_debug_set_fallback_counter(unsigned long long* counter) {
     t_fallback_counter = counter;
     return GRX_OK;

@@ -25,6 +25,10 @@ cudaError_t launch_con2prim(const double* cons, const double* met, long long nc,
                             unsigned long long* nfail, cudaStream_t st);
 cudaError_t launch_rk_axpy(const RhsParams& geom, double a, const double* x, double b, double dt, const double* rhs,
                            double* y, cudaStream_t st);
+cudaError_t launch_rk_stage(const RhsParams& geom, double a, const double* Ua, double b, const double* Ub, double h,
+                            const double* L, double* Uout, double* acc, double wdt, double* prim, unsigned long long* nfail,
+                            cudaStream_t st);
+cudaError_t launch_fill_ghosts(const RhsParams& geom, double* prim, int bc, cudaStream_t st);
 cudaError_t launch_selftest_math(const double* x, double* y, size_t n, cudaStream_t st);
 cudaError_t launch_dfma_peak(int iters, double* sink, double* flops_out, cudaStream_t st);
 

@@ -58,6 +58,62 @@ __global__ void __launch_bounds__(128) rk_axpy_kernel(const __grid_constant__ Rh
     }
 }
 
+// NEXT-1: one Runge-Kutta stage on the interior cells, fused with con2prim:
+//   U_out = a U_a + b (U_b + h L);   acc += wdt L (RK4 only);   prim = con2prim(U_out).
+__global__ void __launch_bounds__(128) rk_stage_kernel(const __grid_constant__ RhsParams p, double a, const double* Ua, double b,
+                                                       const double* Ub, double h, const double* __restrict__ L,
+                                                       double* Uout, double* acc, double wdt, double* __restrict__ prim,
+                                                       unsigned long long* nfail) {
+    const int nxb = (p.n[0] + 127) / 128;
+    const int i = (blockIdx.x % nxb) * 128 + threadIdx.x;
+    const int row = blockIdx.x / nxb;
+    const int j = row % p.n[1], k = row / p.n[1];
+    if (i >= p.n[0]) return;
+    const long long c0 = (i + p.g) + p.stride[1] * (j + p.g) + p.stride[2] * (k + p.g);
+    const long long ub = (long long)blockIdx.y * 8 * p.nc + c0;
+    const double* mb = p.met + (long long)blockIdx.y * 10 * p.nc + c0;
+    double U[8], P[8], m[10];
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const long long o = ub + c * p.nc;
+        const double l = L[o];
+        U[c] = a * Ua[o] + b * (Ub[o] + h * l);
+        Uout[o] = U[c];
+        if (acc) acc[o] += wdt * l;
+    }
+#pragma unroll
+    for (int f = 0; f < 10; ++f) m[f] = mb[f * p.nc];
+    const int bad = con2prim_point(U, m, p.gamma, P);
+#pragma unroll
+    for (int c = 0; c < 8; ++c) prim[ub + c * p.nc] = P[c];
+    if (bad && nfail) atomicAdd(nfail, 1ULL);
+}
+
+// NEXT-1: ghost fill of the 8 primitives at the outer boundary of every box (l.170, l.255, l.329): a ghost cell takes the
+// interior cell whose index is its own, clamped (bc = 0, "copy") or wrapped (bc = 1, periodic) direction by direction.
+__global__ void __launch_bounds__(256) fill_ghosts_kernel(const __grid_constant__ RhsParams p, double* prim, int bc) {
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= p.nc) return;
+    const int I = (int)(c % p.N[0]), J = (int)((c / p.N[0]) % p.N[1]), Kz = (int)(c / p.stride[2]);
+    int s[3] = {I - p.g, J - p.g, Kz - p.g};
+    bool ghost = false;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const int n = p.n[d];
+        int v = s[d];
+        if (v < 0 || v >= n) {
+            ghost = true;
+            v = bc == 1 ? ((v % n) + n) % n : (v < 0 ? 0 : n - 1);
+        }
+        s[d] = v;
+    }
+    if (!ghost) return;
+    const long long src = (s[0] + p.g) + p.stride[1] * (s[1] + p.g) + p.stride[2] * (s[2] + p.g);
+    double* pb = prim + (long long)blockIdx.y * 8 * p.nc;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) pb[q * p.nc + c] = pb[q * p.nc + src];
+}
+
 __global__ void selftest_math_kernel(const double* __restrict__ x, double* __restrict__ y, size_t n) {
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n) return;
@@ -106,6 +162,20 @@ cudaError_t launch_rk_axpy(const RhsParams& p, double a, const double* x, double
                            double* y, cudaStream_t st) {
     const dim3 grid((unsigned)((p.n[0] + 127) / 128) * (unsigned)p.n[1] * (unsigned)p.n[2], p.nbox);
     rk_axpy_kernel<<<grid, 128, 0, st>>>(p, a, x, b, dt, rhs, y);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rk_stage(const RhsParams& p, double a, const double* Ua, double b, const double* Ub, double h,
+                            const double* L, double* Uout, double* acc, double wdt, double* prim, unsigned long long* nfail,
+                            cudaStream_t st) {
+    const dim3 grid((unsigned)((p.n[0] + 127) / 128) * (unsigned)p.n[1] * (unsigned)p.n[2], p.nbox);
+    rk_stage_kernel<<<grid, 128, 0, st>>>(p, a, Ua, b, Ub, h, L, Uout, acc, wdt, prim, nfail);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fill_ghosts(const RhsParams& p, double* prim, int bc, cudaStream_t st) {
+    const dim3 grid((unsigned)((p.nc + 255) / 256), p.nbox);
+    fill_ghosts_kernel<<<grid, 256, 0, st>>>(p, prim, bc);
     return cudaGetLastError();
 }
 

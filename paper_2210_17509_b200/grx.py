@@ -17,7 +17,8 @@ LIB_PATH = os.path.join(_HERE, "libgrx.so")
 RECON = {"minmod": 0, "mc": 1, "weno5": 2}
 VARIANT = {"auto": 0, "simple": 1, "ldg": 2, "tma": 3}
 EXPORTS = (
-    "grx_valencia_rhs", "grx_valencia_rhs_host", "grx_host_workspace_bytes", "grx_prim2con", "grx_con2prim", "grx_rk_axpy", "grx_debug_set_fallback_counter",
+    "grx_valencia_rhs", "grx_valencia_rhs_host", "grx_host_workspace_bytes", "grx_prim2con", "grx_con2prim", "grx_rk_axpy",
+    "grx_step_rk", "grx_step_workspace_bytes", "grx_debug_set_fallback_counter",
     "grx_set_variant", "grx_selftest_math", "grx_dfma_peak_launch", "grx_last_error", "grx_version",
     "grx_weno_eps", "grx_v2max",
 )
@@ -51,6 +52,8 @@ def lib():
         L.grx_prim2con.argtypes = [gp, vp, vp, i, dbl, vp, vp]
         L.grx_con2prim.argtypes = [gp, vp, vp, i, dbl, vp, vp, vp]
         L.grx_rk_axpy.argtypes = [gp, i, dbl, vp, dbl, dbl, vp, vp, vp]
+        L.grx_step_workspace_bytes.argtypes = [gp, i, i]
+        L.grx_step_rk.argtypes = [gp, vp, vp, vp, vp, d3, i, i, dbl, dbl, i, i, i, vp, sz, vp, vp]
         L.grx_debug_set_fallback_counter.argtypes = [vp]
         L.grx_set_variant.argtypes = [i]
         L.grx_selftest_math.argtypes = [vp, vp, sz, vp]
@@ -58,6 +61,7 @@ def lib():
         for name in EXPORTS:
             getattr(L, name).restype = C.c_int
         L.grx_host_workspace_bytes.restype = sz
+        L.grx_step_workspace_bytes.restype = sz
         L.grx_last_error.restype = C.c_char_p
         L.grx_weno_eps.restype = dbl
         L.grx_v2max.restype = dbl
@@ -161,6 +165,34 @@ def rk_axpy(a, x, b, dt, rhs, y, nghost, stream=None):
     _check(lib().grx_rk_axpy(C.byref(g), int(nghost), float(a), _dev(x, 8), float(b), float(dt), _dev(rhs, 8),
                              _dev(y, 8), _stream(stream)))
     return y
+
+
+BC = {"copy": 0, "periodic": 1}
+
+
+def step_workspace_bytes(shape, nghost, rk):
+    nbox, _, Nz, Ny, Nx = shape
+    g = grx_grid(Nx - 2 * nghost, Ny - 2 * nghost, Nz - 2 * nghost, nbox)
+    return lib().grx_step_workspace_bytes(C.byref(g), int(nghost), int(rk))
+
+
+def step_rk(cons, prim, metric, K, dx, nghost, recon, gamma, dt, nsteps, rk=2, bc="copy", workspace=None, nfail=None,
+            stream=None):
+    """grx_step_rk: `nsteps` device-resident method-of-lines steps (in place in cons and prim).  `workspace`: CUDA tensor
+    of at least step_workspace_bytes(...) bytes (allocated if not given)."""
+    import torch
+    g = _grid(prim, nghost)
+    need = step_workspace_bytes(prim.shape, nghost, rk)
+    if workspace is None:
+        workspace = torch.empty(need // 8, dtype=torch.float64, device=prim.device)
+    r = RECON[recon] if isinstance(recon, str) else int(recon)
+    dxa = (C.c_double * 3)(*[float(v) for v in dx])
+    nf = C.c_void_p(nfail.data_ptr()) if nfail is not None else C.c_void_p(0)
+    _check(lib().grx_step_rk(C.byref(g), _dev(cons, 8), _dev(prim, 8), _dev(metric, 10), _dev(K, 6), dxa, int(nghost), r,
+                             float(gamma), float(dt), int(rk), BC[bc] if isinstance(bc, str) else int(bc), int(nsteps),
+                             C.c_void_p(workspace.data_ptr()), workspace.numel() * workspace.element_size(), nf,
+                             _stream(stream)))
+    return cons, prim
 
 
 def set_fallback_counter(counter):

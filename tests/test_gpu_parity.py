@@ -361,6 +361,49 @@ def test_balsara1_rk2_20_steps_gpu_vs_oracle(grx, oracle):
     assert np.abs(y.cpu().numpy()[ii] - expect).max() <= 1e-14 * np.abs(expect).max()
 
 
+@pytest.mark.parametrize("case", ["balsara1-rk2-copy", "balsara1-rk4-copy", "wave-rk4-periodic", "gen-rk2-periodic"])
+def test_device_resident_steps_vs_oracle_loop(grx, oracle, case):
+    """NEXT-1: N method-of-lines steps entirely on the device (grx_step_rk: RHS, stage update fused with con2prim, ghost
+    fill; no host round trip) against the same loop of the oracle (oracle_evolve): 1e-10 max|U| per component (R22)."""
+    import torch
+    from test_oracle_evolve import _periodic_wave
+    if case.startswith("balsara1"):
+        prob, recon, nsteps, cfl = inputs.balsara1(), "minmod", 20, 0.4     # config 1: 20 steps, dt = 0.4 dx (R21)
+    elif case.startswith("wave"):
+        prob, recon, nsteps, cfl = _periodic_wave(24), "weno5", 6, 0.3
+    else:
+        prob, recon, nsteps, cfl = inputs.general_metric_box(n=(20, 12, 10), seed=9, nbox=2), "weno5", 4, 0.2
+    rk = 4 if "rk4" in case else 2
+    bc = "periodic" if "periodic" in case else "copy"
+    dt = cfl * min(prob.dx)
+    prim0 = prob.prim.copy()
+    if not case.startswith("wave"):
+        # the generated ghosts are analytic: refill them the way the loop will, so that both sides start from the same state
+        from evolve import fill_copy_bc
+        g = prob.nghost
+        if bc == "copy":
+            fill_copy_bc(prim0, g)
+        else:
+            ii = np.arange(-g, prob.n[0] + g) % prob.n[0] + g
+            jj = np.arange(-g, prob.n[1] + g) % prob.n[1] + g
+            kk = np.arange(-g, prob.n[2] + g) % prob.n[2] + g
+            prim0 = np.ascontiguousarray(prim0[:, :, kk][:, :, :, jj][:, :, :, :, ii])
+    p_ref, U_ref, nf_ref = oracle.evolve(prim0, prob.metric, prob.K, prob.dx, prob.nghost, recon, prob.gamma, dt, nsteps,
+                                         rk=rk, bc=bc)
+    assert nf_ref == 0
+    prim = torch.from_numpy(prim0).cuda()
+    met, K = torch.from_numpy(prob.metric).cuda(), torch.from_numpy(prob.K).cuda()
+    cons = grx.prim2con(prim, met, prob.nghost, prob.gamma)
+    nfail = torch.zeros(1, dtype=torch.int64, device="cuda")
+    grx.step_rk(cons, prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, dt, nsteps, rk=rk, bc=bc, nfail=nfail)
+    torch.cuda.synchronize()
+    assert int(nfail.item()) == 0
+    ii = prob.interior
+    assert relerr_per_component(cons.cpu().numpy()[ii], U_ref[ii]).max() < 1e-10
+    # primitives incl. their ghost zones follow
+    assert np.abs(prim.cpu().numpy() - p_ref).max() < 1e-9 * np.abs(p_ref).max()
+
+
 def test_selftest_math_accuracy(grx):
     """The MUFU-seeded reciprocal, rsqrt and sqrt helpers are accurate to a few ulp over the range the
     kernels use them on."""
