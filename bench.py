@@ -53,25 +53,27 @@ FLOPS_SURVEY = {"weno5": 4085.0, "minmod": 2140.0}
 # thread instructions per cell.  They belong to ONE state of the kernel sources: `csrc_sha` is the hash of
 # paper_2210_17509_b200/csrc/ they were captured at, and bench.py reports them only while the hash still matches.
 NCU_CAPTURE = {
-    "csrc_sha": "PENDING",
+    "csrc_sha": "d50267afb86c",
     "source": "profiles/r2_ncu_tma.md",
-    "c5-256/weno5/auto": {"traffic": None, "pipe_fp64_pct": None, "fp64_inst_per_cell": None},
-    "c5-256/minmod/auto": {"traffic": None, "pipe_fp64_pct": None, "fp64_inst_per_cell": None},
+    "c5-256/weno5/auto": {"traffic": 4.672716e9, "pipe_fp64_pct": 59.58, "fp64_inst_per_cell": 2636.0},
+    "c5-256/minmod/auto": {"traffic": 4.610271e9, "pipe_fp64_pct": 48.34, "fp64_inst_per_cell": 1357.0},
 }
 KERNEL_OF_VARIANT = {"auto": "rhs_tma_kernel (rhs_fused_kernel for odd Nx)", "tma": "rhs_tma_kernel", "ldg": "rhs_fused_kernel",
                      "simple": "rhs_simple_kernel"}
 SWEEP_POINTS = ("c5-32", "c5-64", "c5-128", "c5-256", "c3", "c4")
 
 
+KERNEL_SOURCES = ("grx_tma.cu", "grx_math.cuh", "grx_common.cuh")   # what the kernel of a step is compiled from
+
+
 def csrc_sha():
-    """Hash of the kernel sources (what NCU_CAPTURE is keyed on)."""
+    """Hash of the sources of the product kernel (what NCU_CAPTURE is keyed on)."""
     import hashlib
     h = hashlib.sha1()
     d = os.path.join(ROOT, "paper_2210_17509_b200", "csrc")
-    for f in sorted(os.listdir(d)):
-        if f.endswith((".cu", ".cuh", ".h")):
-            h.update(f.encode())
-            h.update(open(os.path.join(d, f), "rb").read())
+    for f in KERNEL_SOURCES:
+        h.update(f.encode())
+        h.update(open(os.path.join(d, f), "rb").read())
     return h.hexdigest()[:12]
 
 
@@ -277,6 +279,33 @@ def time_rhs(grx, torch, prob, dev, recon, steps, warmup, stream):
     return e0.elapsed_time(e1) * 1e-3, out
 
 
+def time_zone_cycles(grx, torch, prob, dev, recon, stream, nsteps=5):
+    """zone-cycles/s = steps x cells / time of grx_step_rk: SSP-RK2, periodic ghost fill, every stage =
+    RHS + update fused with con2prim + ghost fill, all on the device."""
+    prim0, met, K = dev
+    prim = prim0.clone()
+    grx_bc = "periodic"
+    cons = grx.prim2con(prim, met, prob.nghost, prob.gamma)
+    ws = torch.empty(grx.step_workspace_bytes(prim.shape, prob.nghost, 2) // 8, dtype=torch.float64, device="cuda")
+    nfail = torch.zeros(1, dtype=torch.int64, device="cuda")
+    dt = 0.2 * min(prob.dx)
+    grx.step_rk(cons, prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, dt, 1, rk=2, bc=grx_bc, workspace=ws, nfail=nfail,
+                stream=stream)      # warm-up step; also makes the ghosts periodic
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stream.synchronize()
+    e0.record(stream)
+    grx.step_rk(cons, prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, dt, nsteps, rk=2, bc=grx_bc, workspace=ws,
+                nfail=nfail, stream=stream)
+    e1.record(stream)
+    stream.synchronize()
+    t = e0.elapsed_time(e1) * 1e-3
+    ok = bool(torch.isfinite(cons[prob.interior]).all().item())
+    return {"value": prob.cells * nsteps / t, "unit": "zone-cycles/s", "steps": nsteps, "ms_per_step": 1e3 * t / nsteps,
+            "scheme": f"SSP-RK2, {recon}+HLLE, Gamma-law con2prim, periodic ghosts, static metric; {prob.name}",
+            "con2prim_failures": int(nfail.item()), "finite": ok,
+            "paper_context": "setupA 0.47e8 zone-cycles/s at 240^3 on one V100 (PAPER.md l.341): other hardware, context only"}
+
+
 def measure_dfma_peak(grx, torch, stream):
     sink = torch.zeros(1, dtype=torch.float64, device="cuda")
     grx.dfma_peak_launch(2000, sink, stream)
@@ -413,6 +442,12 @@ def run_ours(args):
     if not args.no_sweep and args.workload == "c5-256":
         sweep = sweep_points(grx, torch, stream, SWEEP_POINTS, 10, 3, peaks, keep=("c5-256", prob, dev))
 
+    # ---- NEXT-1: device-resident time steps on the same block (context: the paper's setupA, l.329-341: static spacetime,
+    # ideal gas, RK2, WENO5, periodic boundaries, 3 ghosts -> 0.47e8 zone-cycles/s at 240^3 on one V100)
+    zone_cycles = None
+    if not args.no_sweep:
+        zone_cycles = time_zone_cycles(grx, torch, prob, dev, recon, stream)
+
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -430,6 +465,8 @@ def run_ours(args):
     }
     if sweep is not None:
         line["sweep"] = sweep
+    if zone_cycles is not None:
+        line["zone_cycles"] = zone_cycles
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()
