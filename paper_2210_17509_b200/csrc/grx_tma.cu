@@ -137,7 +137,7 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
     using L = Lay<RECON, TY>;
     constexpr int H = L::H, PW = L::PW, PF = L::PF, MH = L::MH, MW = L::MW, MF = L::MF, NT = L::NT, EF = L::EF;
     constexpr unsigned FULL = 0xffffffffu;
-    static_assert(2 * TY <= 32, "the rim warp needs two lanes per row");
+    static_assert(4 * TY <= 32, "the rim warp needs four lanes per row");
     extern __shared__ __align__(1024) double sm[];
     double* const PS = sm + L::o_ps;
     double* const MS = sm + L::o_ms;
@@ -398,24 +398,25 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
         }
     } else {
         // ------------------------------------------------ rim warp: the tile's edge faces, and the TMA producer
-        // x-rim: lane l < tye          -> the first face of row l (between cells X0-1 and X0)
-        //        lane TY + l, l < tye  -> the last face of row l  (between cells X0+txe-1 and X0+txe)
-        // y-rim: lane l < txe          -> cell (X0+l, Y0-1) [q^+ for the row warps] and the last face of column l
-        const bool xl = lane < tye;
-        const bool xr = lane >= TY && (lane - TY) < tye;
-        const int xrow = xl ? lane : lane - TY;
+        // y-rim: lane l < txe -> cell (X0+l, Y0-1) [q^+ for the row warps] and the last face of column l
+        // x-rim lanes, four per row: group 0 = cell X0-1, 1 = X0 (the two sides of the row's first face), 2 = X0+txe-1,
+        // 3 = X0+txe (its last face); one reconstruction pass covers all four, q^- moves from the odd groups to the
+        // even ones by shuffle, and the even groups evaluate the faces
+        const int xgrp = lane / TY, xrow = lane - xgrp * TY;
+        const bool xrec = (xgrp < 4) && (xrow < tye);
+        const bool xface = xrec && !(xgrp & 1);
         const bool ycol = lane < txe;
         // the last faces are the first faces of the next tile too: they count only at the block's end
-        const bool count_x = xl || (X0 + txe == p.n[0]), count_y = (Y0 + tye == p.n[1]);
+        const bool count_x = (xgrp == 0) || (X0 + txe == p.n[0]), count_y = (Y0 + tye == p.n[1]);
         unsigned dup = 0;
-        // staged positions: the cell left of the x-rim face of row xrow, the y-rim cells of column `lane`
-        const int xcol = xl ? -1 : txe - 1;
+        // staged positions: this lane's x-rim cell, the y-rim cells of column `lane`
+        const int xcol = (xgrp == 0) ? -1 : (xgrp == 1) ? 0 : (xgrp == 2) ? txe - 1 : txe;
         const double* const px = PS + (H + xrow) * PW + (H + dP + xcol);
-        const double* const mx = MS + (MH + xrow) * MW + (MH + dM + xcol + 1);
+        const double* const mx = MS + (MH + xrow) * MW + (MH + dM + xcol + 1);   // right cell of the face (even groups)
         const double* const pyb = PS + (H - 1) * PW + (H + dP + lane);
         const double* const pyt = PS + (H + tye) * PW + (H + dP + lane);
         const double* const myt = MS + (MH + tye) * MW + (MH + dM + lane);
-        double* const fxo = FX + (xl ? 0 : 8 * TY) + xrow;
+        double* const fxo = FX + (xgrp == 0 ? 0 : 8 * TY) + xrow;
         for (int kk = -1; kk <= nk; ++kk) {
             mbar_wait(barP, (unsigned)(kk + 1) & 1u);
             if (kk < 0 || kk >= nk) {
@@ -427,18 +428,7 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
                 continue;
             }
             const long long cp = cbase + sz * (kk + 1);   // tile origin in plane k0+kk
-            mbar_wait(barM, (unsigned)kk & 1u);
-            if (xl || xr) {
-                double PL[8], PR[8], tmp[8], Fh[8];
-                recon8_smem<RECON, PF, 1>(px, tmp, PL);
-                recon8_smem<RECON, PF, 1>(px + 1, PR, tmp);
-                FaceGeom m;
-                face_geom_smem<MF, 1>(mx, m);
-                const long long cxr = cp + sy * xrow + xcol + 1;
-                face_flux<0>(m, PL, PR, prim + cxr - 1, prim + cxr, nc, gamma, Fh, count_x ? nfb : dup);
-#pragma unroll
-                for (int q = 0; q < 8; ++q) fxo[q * TY] = Fh[q];
-            }
+            // y first: it needs the staged primitives only; the staged metric (x-rim faces) was requested last
             double yt_qm[8];
             if (ycol) {
                 double tmp[8], yb_qp[8];
@@ -446,6 +436,24 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
 #pragma unroll
                 for (int q = 0; q < 8; ++q) QF[q * EF + lane] = yb_qp[q];
                 recon8_smem<RECON, PF, PW>(pyt, yt_qm, tmp);
+            }
+            mbar_wait(barM, (unsigned)kk & 1u);
+            {
+                double PL[8], PR[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) PL[q] = PR[q] = 0.0;
+                if (xrec) recon8_smem<RECON, PF, 1>(px, PR, PL);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) PR[q] = __shfl_down_sync(FULL, PR[q], TY);   // q^- of the cell to the right
+                if (xface) {
+                    double Fh[8];
+                    FaceGeom m;
+                    face_geom_smem<MF, 1>(mx, m);
+                    const long long cxr = cp + sy * xrow + xcol + 1;
+                    face_flux<0>(m, PL, PR, prim + cxr - 1, prim + cxr, nc, gamma, Fh, count_x ? nfb : dup);
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) fxo[q * TY] = Fh[q];
+                }
             }
             __syncthreads();                                   // (A)
             if (producer) {   // every read of the staged primitives is done: bring in the next plane
