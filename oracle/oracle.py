@@ -50,6 +50,10 @@ def lib():
         L.oracle_sources_point.restype = None
         L.oracle_count_piece.argtypes = [C.c_int, C.c_int, C.c_int, up]
         L.oracle_count_piece.restype = C.c_int
+        L.oracle_face_bfluxes.argtypes = [ip, C.c_int, dp, dp, C.c_int, C.c_int, C.c_double, dp]
+        L.oracle_face_bfluxes.restype = C.c_int
+        L.oracle_flux_ct.argtypes = [ip, C.c_int, dp, dp, C.c_int, dp]
+        L.oracle_flux_ct.restype = C.c_int
         L.oracle_weno_eps.restype = C.c_double
         L.oracle_v2max.restype = C.c_double
         _lib = L
@@ -115,6 +119,38 @@ def con2prim(cons, metric, nghost, gamma):
     if nfail < 0:
         raise ValueError("oracle: invalid argument")
     return prim, nfail
+
+
+def face_bfluxes(prim, metric, nghost, recon, gamma):
+    """NEXT-2: HLLE fluxes of calB on the faces (normal index 0..n, transverse -1..n), FB[nbox, 9, Nz, Ny, Nx] indexed by
+    the cell whose low face it is: FB[:, 3 d + c] = F^d(calB^c); NaN where not defined."""
+    prim, metric = _arr(prim), _arr(metric)
+    n, nbox = _grid(prim, nghost)
+    FB = np.full((nbox, 9) + prim.shape[2:], np.nan)
+    r = RECON[recon] if isinstance(recon, str) else int(recon)
+    if lib().oracle_face_bfluxes(n, nbox, _p(prim), _p(metric), nghost, r, gamma, _p(FB)):
+        raise ValueError("oracle: invalid argument")
+    return FB
+
+
+def flux_ct(FB, dx, nghost):
+    """NEXT-2: d calB^i/dt on the interior cells from the face fluxes by flux-CT (reading R30); dB[nbox, 3, Nz, Ny, Nx],
+    ghost cells NaN."""
+    FB = _arr(FB)
+    nbox, nf, Nz, Ny, Nx = FB.shape
+    n = (C.c_int * 3)(Nx - 2 * nghost, Ny - 2 * nghost, Nz - 2 * nghost)
+    dB = np.full((nbox, 3, Nz, Ny, Nx), np.nan)
+    if lib().oracle_flux_ct(n, nbox, _p(FB), (C.c_double * 3)(*dx), nghost, _p(dB)):
+        raise ValueError("oracle: invalid argument")
+    return dB
+
+
+def valencia_rhs_ct(prim, metric, K, dx, nghost, recon, gamma):
+    """Right-hand side with the calB components replaced by the flux-CT update (NEXT-2)."""
+    out, nfb = valencia_rhs(prim, metric, K, dx, nghost, recon, gamma)
+    dB = flux_ct(face_bfluxes(prim, metric, nghost, recon, gamma), dx, nghost)
+    out[:, 5:8] = dB
+    return out, nfb
 
 
 BC = {"copy": 0, "periodic": 1}

@@ -568,6 +568,107 @@ void fill_ghosts_box(const Grid& G, double* prim, int bc) {
                 }
 }
 
+// ---- NEXT-2: constrained transport for the cell-centred calB^i, reading R30 ------------------
+// The paper evolves the magnetic field with constrained transport in every multi-dimensional test (l.287, l.299, l.315)
+// and names the staggered face / edge locations it lives on (l.194-196), but prints no algorithm (ref [56] is not in the
+// reference).  R30 takes the flux-CT scheme that can be stated from the induction equation alone: the HLLE fluxes of
+// calB are minus / plus the electromotive force, F^j(calB^i) = eps_{ijk} E_k (d_t B = -curl E), i.e.
+//     F^x(B^y) = -E_z   F^y(B^x) = +E_z      F^y(B^z) = -E_x   F^z(B^y) = +E_x      F^z(B^x) = -E_y   F^x(B^z) = +E_y.
+// (1) the face fluxes are evaluated exactly as in the right-hand side (same reconstruction, face metric, HLLE), also on the
+//     one layer of grid lines next to the block (transverse index -1 and n), which the edge averages below reach;
+// (2) the EMF on a cell EDGE is the arithmetic mean of the four face fluxes that touch the edge, with those signs;
+// (3) the flux of calB^i through a face is replaced by the mean of the two edge EMFs on that face, and d calB^i/dt is the
+//     difference of those replaced fluxes -- a discrete curl of edge EMFs, so the vertex-centred divergence (at a vertex:
+//     sum_d [mean of B^d over the four cells on the high side - mean over the four on the low side] / dx_d) of the update
+//     vanishes to rounding wherever the eight cells around the vertex are updated.
+// FB layout: [9][Nz][Ny][Nx] per box, FB[3 d + c] = F^d(calB^c) at the LOW d-face of the cell it is indexed by (face
+// i-1/2 for d = x, ...); normal index 0..n, transverse indices -1..n; other entries untouched.  The three normal
+// components F^d(calB^d) -- the purely dissipative part of the HLLE flux, which flux-CT drops -- are stored so that the
+// pins can rebuild the plain right-hand side from FB.
+void face_bflux_box(const Grid& G, const double* prim, const double* met, int recon, double gamma_d, double* FB) {
+    const size_t NC = G.ncell;
+    for (int d = 0; d < 3; ++d) {
+        const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+        const int nd = G.n[d], n1 = G.n[d1] + 2, n2 = G.n[d2] + 2;
+#pragma omp parallel
+        {
+            unsigned long long nfb = 0;
+            std::vector<double> qm(8 * (size_t)(nd + 2)), qp(8 * (size_t)(nd + 2));
+#pragma omp for schedule(static)
+            for (long line = 0; line < (long)n1 * n2; ++line) {
+                int ijk[3];
+                ijk[d1] = (int)(line % n1) - 1;
+                ijk[d2] = (int)(line / n1) - 1;
+                auto at = [&](int s) {
+                    int c3[3] = {ijk[0], ijk[1], ijk[2]};
+                    c3[d] = s;
+                    return G.idx(c3[0], c3[1], c3[2]);
+                };
+                for (int s = -1; s <= nd; ++s)
+                    for (int q = 0; q < 8; ++q) {
+                        const double* f = prim + q * NC;
+                        const double a = (recon == RECON_WENO5) ? f[at(s - 2)] : 0.0;
+                        const double e = (recon == RECON_WENO5) ? f[at(s + 2)] : 0.0;
+                        recon_cell<double>(recon, a, f[at(s - 1)], f[at(s)], f[at(s + 1)], e, qm[q * (nd + 2) + s + 1],
+                                           qp[q * (nd + 2) + s + 1]);
+                    }
+                for (int f = 0; f <= nd; ++f) {
+                    const size_t iL = at(f - 1), iR = at(f);
+                    Metric<double> mf;
+                    mf.alp = 0.5 * (met[0 * NC + iL] + met[0 * NC + iR]);
+                    for (int i = 0; i < 3; ++i) mf.beta[i] = 0.5 * (met[(1 + i) * NC + iL] + met[(1 + i) * NC + iR]);
+                    for (int c = 0; c < 6; ++c) mf.g[c] = 0.5 * (met[(4 + c) * NC + iL] + met[(4 + c) * NC + iR]);
+                    double PL[8], PR[8], CL[8], CR[8], Fh[8];
+                    for (int q = 0; q < 8; ++q) {
+                        PL[q] = qp[q * (nd + 2) + f];
+                        PR[q] = qm[q * (nd + 2) + f + 1];
+                        CL[q] = prim[q * NC + iL];
+                        CR[q] = prim[q * NC + iR];
+                    }
+                    face_flux(mf, d, gamma_d, PL, PR, CL, CR, Fh, &nfb);
+                    for (int c = 0; c < 3; ++c) FB[(3 * d + c) * NC + iR] = Fh[5 + c];
+                }
+            }
+        }
+    }
+    t_ops = {0, 0, 0, 0};
+}
+
+// Steps (2) and (3): d calB^i / dt on the interior cells from the face fluxes FB.
+void flux_ct_box(const Grid& G, const double* FB, const double dx[3], double* dB) {
+    const size_t NC = G.ncell;
+    const double* FxBy = FB + 1 * NC; const double* FxBz = FB + 2 * NC;
+    const double* FyBx = FB + 3 * NC; const double* FyBz = FB + 5 * NC;
+    const double* FzBx = FB + 6 * NC; const double* FzBy = FB + 7 * NC;
+    // edge EMFs, indexed by the cell whose LOW-LOW edge it is: Ez(i,j,k) sits at (i-1/2, j-1/2, k), and so on
+    auto Ez = [&](int i, int j, int k) {
+        return 0.25 * (-FxBy[G.idx(i, j, k)] - FxBy[G.idx(i, j - 1, k)] + FyBx[G.idx(i, j, k)] + FyBx[G.idx(i - 1, j, k)]);
+    };
+    auto Ex = [&](int i, int j, int k) {
+        return 0.25 * (-FyBz[G.idx(i, j, k)] - FyBz[G.idx(i, j, k - 1)] + FzBy[G.idx(i, j, k)] + FzBy[G.idx(i, j - 1, k)]);
+    };
+    auto Ey = [&](int i, int j, int k) {
+        return 0.25 * (-FzBx[G.idx(i, j, k)] - FzBx[G.idx(i - 1, j, k)] + FxBz[G.idx(i, j, k)] + FxBz[G.idx(i, j, k - 1)]);
+    };
+#pragma omp parallel for schedule(static) collapse(2)
+    for (int k = 0; k < G.n[2]; ++k)
+        for (int j = 0; j < G.n[1]; ++j)
+            for (int i = 0; i < G.n[0]; ++i) {
+                // replaced fluxes on the six faces of the cell: mean of the two edge EMFs on the face, with the sign of
+                // F^j(B^i) = eps_{ijk} E_k
+                const double FyBx_lo = 0.5 * (Ez(i, j, k) + Ez(i + 1, j, k)), FyBx_hi = 0.5 * (Ez(i, j + 1, k) + Ez(i + 1, j + 1, k));
+                const double FzBx_lo = -0.5 * (Ey(i, j, k) + Ey(i + 1, j, k)), FzBx_hi = -0.5 * (Ey(i, j, k + 1) + Ey(i + 1, j, k + 1));
+                const double FxBy_lo = -0.5 * (Ez(i, j, k) + Ez(i, j + 1, k)), FxBy_hi = -0.5 * (Ez(i + 1, j, k) + Ez(i + 1, j + 1, k));
+                const double FzBy_lo = 0.5 * (Ex(i, j, k) + Ex(i, j + 1, k)), FzBy_hi = 0.5 * (Ex(i, j, k + 1) + Ex(i, j + 1, k + 1));
+                const double FxBz_lo = 0.5 * (Ey(i, j, k) + Ey(i, j, k + 1)), FxBz_hi = 0.5 * (Ey(i + 1, j, k) + Ey(i + 1, j, k + 1));
+                const double FyBz_lo = -0.5 * (Ex(i, j, k) + Ex(i, j, k + 1)), FyBz_hi = -0.5 * (Ex(i, j + 1, k) + Ex(i, j + 1, k + 1));
+                const size_t c = G.idx(i, j, k);
+                dB[0 * NC + c] = -(FyBx_hi - FyBx_lo) / dx[1] - (FzBx_hi - FzBx_lo) / dx[2];
+                dB[1 * NC + c] = -(FxBy_hi - FxBy_lo) / dx[0] - (FzBy_hi - FzBy_lo) / dx[2];
+                dB[2 * NC + c] = -(FxBz_hi - FxBz_lo) / dx[0] - (FyBz_hi - FyBz_lo) / dx[1];
+            }
+}
+
 }  // namespace
 
 // =================================================== C ABI ===================================================
@@ -835,6 +936,32 @@ int oracle_count_piece(int piece, int d, int recon, unsigned long long ops[4]) {
     }
     ops[0] = t_ops.add; ops[1] = t_ops.mul; ops[2] = t_ops.div; ops[3] = t_ops.sqrt;
     t_ops = {0, 0, 0, 0};
+    return 0;
+}
+
+// NEXT-2: face fluxes of calB (FB, [nbox][9][Nz][Ny][Nx]) and the flux-CT update (dB, [nbox][3][Nz][Ny][Nx], interior cells).
+int oracle_face_bfluxes(const int n[3], int nbox, const double* prim, const double* metric, int nghost, int recon,
+                        double gamma, double* FB) {
+    if (!n || !prim || !metric || !FB || nbox < 1 || n[0] < 1 || n[1] < 1 || n[2] < 1) return 1;
+    if (recon != RECON_MINMOD && recon != RECON_MC && recon != RECON_WENO5) return 1;
+    if (nghost < (recon == RECON_WENO5 ? 3 : 2) || !(gamma > 1.0)) return 1;
+    Grid G;
+    for (int a = 0; a < 3; ++a) { G.n[a] = n[a]; G.N[a] = n[a] + 2 * nghost; }
+    G.g = nghost;
+    G.ncell = (size_t)G.N[0] * G.N[1] * G.N[2];
+    for (int b = 0; b < nbox; ++b)
+        face_bflux_box(G, prim + (size_t)b * 8 * G.ncell, metric + (size_t)b * 10 * G.ncell, recon, gamma,
+                       FB + (size_t)b * 9 * G.ncell);
+    return 0;
+}
+
+int oracle_flux_ct(const int n[3], int nbox, const double* FB, const double dx[3], int nghost, double* dB) {
+    if (!n || !FB || !dx || !dB || nbox < 1 || n[0] < 1 || n[1] < 1 || n[2] < 1 || nghost < 1) return 1;
+    Grid G;
+    for (int a = 0; a < 3; ++a) { G.n[a] = n[a]; G.N[a] = n[a] + 2 * nghost; }
+    G.g = nghost;
+    G.ncell = (size_t)G.N[0] * G.N[1] * G.N[2];
+    for (int b = 0; b < nbox; ++b) flux_ct_box(G, FB + (size_t)b * 9 * G.ncell, dx, dB + (size_t)b * 3 * G.ncell);
     return 0;
 }
 
