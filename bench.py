@@ -320,6 +320,30 @@ def measure_dfma_peak(grx, torch, stream):
     return best / 1e12
 
 
+ISSUE_PROBE_MODES = ("dfma_fixed_operands", "dfma_three_registers", "dmul", "dmul+imad", "dmul+sts64", "dmul+shfl")
+
+
+def measure_issue_probe(grx, torch, stream, sm_mhz):
+    """FP64 lanes per clock per SM (64 = nominal) of the issue probe's six patterns (include/grx.h): what an FP64
+    instruction costs with three register operands, and next to integer, store and shuffle instructions."""
+    sink = torch.zeros(1, dtype=torch.float64, device="cuda")
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    hz = (sm_mhz or 1965.0) * 1e6
+    res = {}
+    for mode, name in enumerate(ISSUE_PROBE_MODES):
+        grx.fp64_issue_probe(mode, 500, sink, stream)
+        best = 0.0
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            n = grx.fp64_issue_probe(mode, 4000, sink, stream)
+            e1.record(stream)
+            stream.synchronize()
+            best = max(best, n / (e0.elapsed_time(e1) * 1e-3))
+        res[name] = round(best / hz / sms, 2)
+    return res
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -419,6 +443,7 @@ def run_ours(args):
         "hbm": {"achieved": ach_gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s", "peak_source": peak_src,
                 "frac": ach_gbs / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None},
         "traffic": None,
+        "fp64_lanes_per_clk_per_sm": measure_issue_probe(grx, torch, stream, clocks.get("sm_mhz")),
     }
     # profiler-only numbers: reported only for the state of the kernel sources they were captured at
     sha = csrc_sha()

@@ -377,6 +377,13 @@ int grx_dfma_peak_launch(int iters, double* sink, double* flops_out, void* cuda_
     return GRX_OK;
 }
 
+int grx_fp64_issue_probe(int mode, int iters, double* sink, double* fp64_instr_out, void* cuda_stream) {
+    if (mode < 0 || mode > 5 || iters < 1 || !sink) return fail(GRX_ERR_INVALID_ARG, "mode must be 0..5, iters >= 1 and sink non-NULL");
+    const cudaError_t e = grx::launch_issue_probe(mode, iters, sink, fp64_instr_out, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_fp64_issue_probe");
+    return GRX_OK;
+}
+
 const char* grx_last_error(void) { return t_err; }
 int grx_version(void) { return 100; }   /* 0.1.0 */
 double grx_weno_eps(void) { return grx::WENO_EPS; }

@@ -197,4 +197,61 @@ cudaError_t launch_dfma_peak(int iters, double* sink, double* flops_out, cudaStr
     return cudaGetLastError();
 }
 
+// ---- issue probe: what an FP64 instruction really costs next to its operands and its neighbours ---------------
+// 16 independent values per thread, every instruction reads values written 9 or more instructions earlier, so
+// neither latency nor the reuse cache limits the rate.  MODE 0: a = fma(a, m, c) with m, c fixed (the classic peak loop);
+// 1: DFMA with three distinct, changing register operands; 2: DMUL of two registers; 3: 2 + one independent IMAD per
+// DMUL; 4: 2 + one STS.64 per DMUL; 5: 2 + one SHFL per DMUL.
+constexpr int PROBE_THREADS = 256, PROBE_VALUES = 16;
+template <int MODE>
+__global__ void __launch_bounds__(PROBE_THREADS) issue_probe_kernel(int iters, double* sink) {
+    __shared__ double sh[PROBE_THREADS * 8];
+    double r[PROBE_VALUES];
+    int x[8];
+    const double m = 1.0 - 1e-9 * (threadIdx.x & 7), c = 1e-12 * blockIdx.x;
+#pragma unroll
+    for (int i = 0; i < PROBE_VALUES; ++i) r[i] = 1.0 + 1e-9 * (threadIdx.x + i);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { x[i] = threadIdx.x + i; sh[threadIdx.x + PROBE_THREADS * i] = 1.0; }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < PROBE_VALUES; ++i) {
+            const int j = (i + 1) % PROBE_VALUES, l = (i + 7) % PROBE_VALUES, n = (i + 11) % PROBE_VALUES;
+            if (MODE == 0) r[i] = fma(r[i], m, c);
+            if (MODE == 1) r[i] = fma(r[j], r[l], r[n]);
+            if (MODE >= 2) r[i] = r[j] * r[l];
+            if (MODE == 3) x[i % 8] = x[i % 8] * 5 + x[(i + 3) % 8];
+            if (MODE == 4) sh[threadIdx.x + PROBE_THREADS * (i % 8)] = r[n];
+            if (MODE == 5) x[i % 8] = __shfl_xor_sync(0xffffffffu, x[i % 8], 1);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < PROBE_VALUES; ++i) s += r[i];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i] + sh[(threadIdx.x * 7 + PROBE_THREADS * i) % (PROBE_THREADS * 8)];
+    if (s == 1.2345678) *sink = s;
+}
+
+cudaError_t launch_issue_probe(int mode, int iters, double* sink, double* fp64_instr_out, cudaStream_t st) {
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    const int blocks = sms * 2;   // 2 x 256 threads per SM: 4 warps per scheduler
+    switch (mode) {
+        case 0: issue_probe_kernel<0><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
+        case 1: issue_probe_kernel<1><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
+        case 2: issue_probe_kernel<2><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
+        case 3: issue_probe_kernel<3><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
+        case 4: issue_probe_kernel<4><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
+        case 5: issue_probe_kernel<5><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
+        default: return cudaErrorInvalidValue;
+    }
+    // FP64 thread-instructions of the launch (one per value and iteration)
+    if (fp64_instr_out) *fp64_instr_out = (double)PROBE_VALUES * (double)iters * PROBE_THREADS * (double)blocks;
+    return cudaGetLastError();
+}
+
 }  // namespace grx

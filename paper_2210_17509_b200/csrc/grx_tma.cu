@@ -227,7 +227,8 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
         }
         // The global loads of a step -- the look-ahead plane of the primitives, metric plane k+2 and K_ij -- are issued
         // one step ahead, before the last barrier of the step before, so that they are in flight while the CTA waits
-        // there.  The producer's TMA prefetch has pulled their lines into L2 by then.
+        // there (measured: issuing the metric and K_ij at the top of their own step costs 2-5 %).  The producer's TMA
+        // prefetch has pulled their lines into L2 by then.
         double qn[8], mn[10], K6[6], dz[10];
         auto issue_loads = [&](int kn, long long cn) {
             if (kn <= nk) {
@@ -349,6 +350,9 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
                 for (int q = 0; q < 8; ++q) qf[q * EF + 32] = qx[q];
             }
             __syncthreads();                                   // (A) the staged primitives are free from here on
+            double Fh[8];   // flux of this cell's low y face: published for the row below, kept for the own difference
+#pragma unroll
+            for (int q = 0; q < 8; ++q) Fh[q] = 0.0;
             if (active) {
                 if (first || last) {
                     // x difference of the row's end cells: low face from FX[0] / parked, high face from parked / FX[1]
@@ -380,7 +384,7 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
                     acc[4] += st + sources_K(s, K6);
                 }
                 // ---------------- y face
-                double PL[8], Fh[8];
+                double PL[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) PL[q] = qf[q * EF];
                 FaceGeom m;
@@ -393,7 +397,7 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
             __syncthreads();                                   // (B) the staged metric is free from here on
             if (active) {
 #pragma unroll
-                for (int q = 0; q < 8; ++q) acc[q] = fma(qf[q * EF] - qf[q * EF + 32], p.idx[1], acc[q]);
+                for (int q = 0; q < 8; ++q) acc[q] = fma(Fh[q] - qf[q * EF + 32], p.idx[1], acc[q]);
             }
         }
     } else {
@@ -560,6 +564,7 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
         !make_map(&tmK, p.K, p, 6, TX + 2, TY))
         return cudaErrorNotSupported;
     const size_t smem = (size_t)L::total * sizeof(double);
+    // per device and cheap: set on every launch (no cached state, safe with several devices and host threads)
     // per device and cheap: set on every launch (no cached state, safe with several devices and host threads)
     e = cudaFuncSetAttribute(rhs_tma_kernel<RECON, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

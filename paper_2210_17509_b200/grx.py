@@ -19,7 +19,7 @@ VARIANT = {"auto": 0, "simple": 1, "ldg": 2, "tma": 3}
 EXPORTS = (
     "grx_valencia_rhs", "grx_valencia_rhs_host", "grx_host_workspace_bytes", "grx_prim2con", "grx_con2prim", "grx_rk_axpy",
     "grx_step_rk", "grx_step_workspace_bytes", "grx_debug_set_fallback_counter",
-    "grx_set_variant", "grx_selftest_math", "grx_dfma_peak_launch", "grx_last_error", "grx_version",
+    "grx_set_variant", "grx_selftest_math", "grx_dfma_peak_launch", "grx_fp64_issue_probe", "grx_last_error", "grx_version",
     "grx_weno_eps", "grx_v2max",
 )
 
@@ -58,6 +58,7 @@ def lib():
         L.grx_set_variant.argtypes = [i]
         L.grx_selftest_math.argtypes = [vp, vp, sz, vp]
         L.grx_dfma_peak_launch.argtypes = [i, vp, d3, vp]
+        L.grx_fp64_issue_probe.argtypes = [i, i, vp, d3, vp]
         for name in EXPORTS:
             getattr(L, name).restype = C.c_int
         L.grx_host_workspace_bytes.restype = sz
@@ -218,6 +219,14 @@ def dfma_peak_launch(iters, sink, stream=None):
     flops = C.c_double(0.0)
     _check(lib().grx_dfma_peak_launch(int(iters), _dev(sink), C.byref(flops), _stream(stream)))
     return flops.value
+
+
+def fp64_issue_probe(mode, iters, sink, stream=None):
+    """Launches the FP64 issue probe once in operand pattern `mode` (0..5, include/grx.h); returns the FP64
+    thread-instruction count of the launch."""
+    n = C.c_double(0.0)
+    _check(lib().grx_fp64_issue_probe(int(mode), int(iters), _dev(sink), C.byref(n), _stream(stream)))
+    return n.value
 
 
 def version():

@@ -274,6 +274,76 @@ def test_stream_ordering_and_determinism(grx):
     assert torch.equal(outs[0], outs[1]) and torch.equal(outs[1], outs[2])
 
 
+def test_guard_bands_no_out_of_bounds_access(grx):
+    """Bounds evidence without a sanitizer (compute-sanitizer is closed on this GPU pool): every array of a call sits
+    inside a larger allocation whose guard bands hold NaN (inputs) or a sentinel (out).  A read outside an input array
+    that reaches the arithmetic turns a result into NaN, a write outside `out` changes a guard: the results must be the
+    bits of the plain call and the guards untouched -- for the TMA kernel (whose boxes and L2 prefetches run over the
+    tile edge), the LDG kernel (software prefetch of later planes) and the host entry point's slab calls."""
+    import torch
+    GUARD = 4096          # doubles on each side (32 KB: more than any halo'd row, plane tail or prefetch distance)
+    cases = [(inputs.general_metric_box(n=(34, 9, 11), seed=9, nbox=2), "tma"),
+             (inputs.general_metric_box(n=(30, 16, 40), seed=10, nbox=1), "tma"),
+             (inputs.general_metric_box(n=(33, 12, 9), seed=12, nbox=2), "ldg"),
+             (inputs.general_metric_box(n=(2, 2, 3), seed=13, nbox=1), "auto")]
+    for prob, variant in cases:
+        plain = _to_dev(prob)
+
+        def guarded(a, fill):
+            buf = torch.full((a.numel() + 2 * GUARD,), fill, dtype=torch.float64, device="cuda")
+            view = buf[GUARD:GUARD + a.numel()].view(a.shape)
+            view.copy_(a)
+            return buf, view
+
+        bufs = [guarded(a, float("nan")) for a in plain]
+        obuf = torch.full((plain[0].numel() + 2 * GUARD,), -7.25e300, dtype=torch.float64, device="cuda")
+        out = obuf[GUARD:GUARD + plain[0].numel()].view(plain[0].shape)
+        grx.set_variant(variant)
+        try:
+            for recon in ("minmod", "weno5"):
+                ref = grx.valencia_rhs(*plain, prob.dx, prob.nghost, recon, prob.gamma)
+                obuf.fill_(-7.25e300)
+                grx.valencia_rhs(bufs[0][1], bufs[1][1], bufs[2][1], prob.dx, prob.nghost, recon, prob.gamma, out=out)
+                torch.cuda.synchronize()
+                ii = prob.interior
+                assert torch.equal(out[ii], ref[ii]), f"{prob.name}/{variant}/{recon}: guarded call differs"
+                assert bool((obuf[:GUARD] == -7.25e300).all()) and bool((obuf[-GUARD:] == -7.25e300).all()), \
+                    f"{prob.name}/{variant}/{recon}: a guard band of out was written"
+                for b, _ in bufs:
+                    assert bool(torch.isnan(b[:GUARD]).all()) and bool(torch.isnan(b[-GUARD:]).all())
+        finally:
+            grx.set_variant("auto")
+
+
+def test_repeated_launches_bitwise_under_load(grx):
+    """Race evidence without a sanitizer: the TMA kernel's shared-memory hand-offs (mbarrier-completed TMA planes, two
+    CTA barriers per plane, the rim warp's exchange slots) are exercised 40 times on a ragged multi-tile batch while a
+    second stream keeps the SMs busy with another launch, so that CTAs are scheduled in changing company; every result
+    must be bit-identical to the first."""
+    import torch
+    prob = inputs.general_metric_box(n=(70, 30, 21), seed=17, nbox=3)
+    prim, met, K = _to_dev(prob)
+    big = inputs.sweep_boxes(64, 4)
+    bdev = _to_dev(big)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    grx.set_variant("tma")
+    try:
+        for recon in ("weno5", "minmod"):
+            first = None
+            for it in range(40):
+                if it % 2 == 0:
+                    grx.valencia_rhs(*bdev, big.dx, big.nghost, recon, big.gamma, stream=s2)
+                out = grx.valencia_rhs(prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, stream=s1)
+                s1.synchronize()
+                if first is None:
+                    first = out
+                else:
+                    assert torch.equal(out[prob.interior], first[prob.interior]), f"{recon}: launch {it} differs"
+            s2.synchronize()
+    finally:
+        grx.set_variant("auto")
+
+
 def test_uniform_state_constant_metric_exact_zero(grx):
     """Pin P5 on the GPU: a uniform state on any constant metric has an exactly vanishing right-hand side
     in the flux part and rounding-level sources (the derivative stencil gives exact zeros)."""
