@@ -306,6 +306,26 @@ def time_zone_cycles(grx, torch, prob, dev, recon, stream, nsteps=5):
             "paper_context": "setupA 0.47e8 zone-cycles/s at 240^3 on one V100 (PAPER.md l.341): other hardware, context only"}
 
 
+def time_ct(grx, torch, prob, dev, recon, stream, steps=10):
+    """NEXT-2: grx_valencia_rhs_ct = right-hand side (face fluxes of calB written by the same launch) + face kernel for the
+    lines next to the block + flux-CT kernel."""
+    prim, met, K = dev
+    out = torch.empty_like(prim)
+    ws = torch.empty((prim.shape[0], 6) + tuple(prim.shape[2:]), dtype=torch.float64, device="cuda")
+    for _ in range(3):
+        grx.valencia_rhs_ct(prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, out=out, workspace=ws, stream=stream)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stream.synchronize()
+    e0.record(stream)
+    for _ in range(steps):
+        grx.valencia_rhs_ct(prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, out=out, workspace=ws, stream=stream)
+    e1.record(stream)
+    stream.synchronize()
+    t = e0.elapsed_time(e1) * 1e-3 / steps
+    return {"value": prob.cells / t, "unit": UNIT, "ms_per_call": 1e3 * t, "kernels_per_call": 3,
+            "scheme": f"flux-CT of calB (reading R30), {recon}+HLLE; {prob.name}"}
+
+
 def measure_dfma_peak(grx, torch, stream):
     sink = torch.zeros(1, dtype=torch.float64, device="cuda")
     grx.dfma_peak_launch(2000, sink, stream)
@@ -469,9 +489,10 @@ def run_ours(args):
 
     # ---- NEXT-1: device-resident time steps on the same block (context: the paper's setupA, l.329-341: static spacetime,
     # ideal gas, RK2, WENO5, periodic boundaries, 3 ghosts -> 0.47e8 zone-cycles/s at 240^3 on one V100)
-    zone_cycles = None
+    zone_cycles = ct = None
     if not args.no_sweep:
         zone_cycles = time_zone_cycles(grx, torch, prob, dev, recon, stream)
+        ct = time_ct(grx, torch, prob, dev, recon, stream)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -492,6 +513,8 @@ def run_ours(args):
         line["sweep"] = sweep
     if zone_cycles is not None:
         line["zone_cycles"] = zone_cycles
+    if ct is not None:
+        line["constrained_transport"] = ct
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()

@@ -143,6 +143,22 @@ int grx_step_rk(const grx_grid* grid, double* cons, double* prim, const double* 
                 const double dx[3], int nghost, int recon, double gamma, double dt, int rk_order, int bc, int nsteps,
                 void* workspace, size_t workspace_bytes, unsigned long long* nfail, void* cuda_stream);
 
+/* NEXT-2: the right-hand side with constrained transport for the magnetic field (PAPER.md l.287,
+ * l.299, l.315; face / edge locations l.194-196).  The paper prints no algorithm; reading R30 is flux-CT of the
+ * cell-centred calB^i: with F^j(calB^i) = eps_ijk E_k, the EMF on a cell edge is the mean of the four HLLE face fluxes that
+ * touch it, the flux through a face is replaced by the mean of the two edge EMFs on it, and out[5..7] = d calB^i/dt becomes
+ * the difference of the replaced fluxes (the vertex-centred divergence of the update vanishes to rounding).  out[0..4] are
+ * those of grx_valencia_rhs, bit for bit.  The face fluxes come out of the same kernel launch as the right-hand side (TMA
+ * kernel) plus a kernel for the one layer of grid lines next to the block, whose faces the edge averages reach: prim and
+ * metric must be filled on the ghost cells as for grx_valencia_rhs, no wider.
+ *   workspace  DEVICE pointer, at least grx_ct_workspace_bytes(grid, nghost) bytes (six face-flux arrays), owned by the
+ *              caller; holds F^x(B^y), F^x(B^z), F^y(B^x), F^y(B^z), F^z(B^x), F^z(B^y) at the low face of each cell on return.
+ * Other arguments, return codes and asynchrony as for grx_valencia_rhs. */
+size_t grx_ct_workspace_bytes(const grx_grid* grid, int nghost);
+int grx_valencia_rhs_ct(const grx_grid* grid, const double* prim, const double* metric, const double* K,
+                        const double dx[3], int nghost, int recon, double gamma, double* out, void* workspace,
+                        size_t workspace_bytes, void* cuda_stream);
+
 /* Debug: if `counter` (DEVICE pointer to one unsigned long long, caller-zeroed) is non-NULL, later
  * grx_valencia_rhs calls of this host thread add to it the number of face sides that took the R5
  * first-order fallback.  NULL switches counting off (the default; counting costs a few atomics). */

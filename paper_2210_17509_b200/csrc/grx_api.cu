@@ -47,32 +47,38 @@ const char* make_geom(const grx_grid* grid, int nghost, grx::RhsParams& p) {
     return nullptr;
 }
 
+// Kernel of the product path for this block: 0 = simple, 1 = LDG, 2 = TMA, -1 = TMA forced on arrays it cannot take.
+int choose_kernel(const grx::RhsParams& p, int recon) {
+    const int variant = g_variant.load();
+    if (variant == GRX_VARIANT_SIMPLE) return 0;
+    if (variant == GRX_VARIANT_LDG) return 1;
+    const bool ok = grx::tma_supported(p);
+    if (variant == GRX_VARIANT_TMA) return ok ? 2 : -1;
+    if (!ok) return 1;
+    // AUTO, both kernels take the block: choose by the expected time.  Per cell of a well-filled machine the TMA kernel
+    // is about 1.12x (WENO5) to 1.22x (TVD) faster; on small blocks and batches its 7-row tiles and its per-chunk
+    // set-up fill the SMs less well than the LDG kernel's 11-row tiles (constants fitted on the config-5 sweep,
+    // profiles/r2_sweep.md: the selector picks the faster kernel at every point).
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) {
+        const double gain = (recon == GRX_RECON_WENO5) ? 1.12 : 1.22;
+        if (gain * grx::tma_tile_efficiency(p, sms) < grx::fused_tile_efficiency(p, sms)) return 1;
+    }
+    return 2;
+}
+
 // Launches the selected kernel on a (sub-)block.  `unsupported` is set when the TMA kernel was forced on arrays it
 // cannot take.
 cudaError_t launch_variant(const grx::RhsParams& p, int recon, cudaStream_t st, bool* unsupported = nullptr) {
-    const int variant = g_variant.load();
-    if (variant == GRX_VARIANT_SIMPLE) return grx::launch_rhs_simple(p, recon, st);
-    if (variant == GRX_VARIANT_LDG) return grx::launch_rhs_fused(p, recon, st);
-    const bool ok = grx::tma_supported(p);
-    if (variant == GRX_VARIANT_TMA && !ok) {
-        if (unsupported) *unsupported = true;
-        return cudaErrorNotSupported;
+    switch (choose_kernel(p, recon)) {
+        case 0: return grx::launch_rhs_simple(p, recon, st);
+        case 1: return grx::launch_rhs_fused(p, recon, st);
+        case 2: return grx::launch_rhs_tma(p, recon, 7, st);
+        default:
+            if (unsupported) *unsupported = true;
+            return cudaErrorNotSupported;
     }
-    if (!ok) return grx::launch_rhs_fused(p, recon, st);
-    if (variant == GRX_VARIANT_AUTO) {
-        // Both kernels take the block: choose by the expected time.  Per cell of a well-filled machine the TMA kernel
-        // is about 1.12x (WENO5) to 1.22x (TVD) faster; on small blocks and batches its 7-row tiles and its per-chunk
-        // set-up fill the SMs less well than the LDG kernel's 11-row tiles (constants fitted on the config-5 sweep,
-        // profiles/r2_sweep.md: the selector picks the faster kernel at every point).
-        int dev = 0, sms = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) {
-            const double gain = (recon == GRX_RECON_WENO5) ? 1.12 : 1.22;
-            if (gain * grx::tma_tile_efficiency(p, sms) < grx::fused_tile_efficiency(p, sms))
-                return grx::launch_rhs_fused(p, recon, st);
-        }
-    }
-    return grx::launch_rhs_tma(p, recon, 7, st);
 }
 
 // The two internal streams of grx_valencia_rhs_host: one pair per host thread and device, created on first use.
@@ -282,6 +288,58 @@ int grx_rk_axpy(const grx_grid* grid, int nghost, double a, const double* x, dou
     if (!x || !rhs || !y) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
     const cudaError_t e = grx::launch_rk_axpy(p, a, x, b, dt, rhs, y, static_cast<cudaStream_t>(cuda_stream));
     if (e != cudaSuccess) return fail_cuda(e, "grx_rk_axpy launch");
+    return GRX_OK;
+}
+
+size_t grx_ct_workspace_bytes(const grx_grid* grid, int nghost) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (make_geom(grid, nghost, p)) return 0;
+    return (size_t)6 * (size_t)p.nc * (size_t)p.nbox * sizeof(double);
+}
+
+int grx_valencia_rhs_ct(const grx_grid* grid, const double* prim, const double* metric, const double* K,
+                        const double dx[3], int nghost, int recon, double gamma, double* out, void* workspace,
+                        size_t workspace_bytes, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim || !metric || !K || !dx || !out || !workspace) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (recon != GRX_RECON_MINMOD && recon != GRX_RECON_MC && recon != GRX_RECON_WENO5)
+        return fail(GRX_ERR_INVALID_ARG, "unknown recon");
+    if (nghost < (recon == GRX_RECON_WENO5 ? 3 : 2))
+        return fail(GRX_ERR_INVALID_ARG, "nghost too small: WENO5 needs 3, minmod/MC need 2 (R29)");
+    if (!(gamma > 1.0)) return fail(GRX_ERR_INVALID_ARG, "gamma must be > 1");
+    for (int a = 0; a < 3; ++a) {
+        if (!(dx[a] > 0.0) || !(1.0 / dx[a] > 0.0)) return fail(GRX_ERR_INVALID_ARG, "dx must be > 0 and finite");
+        p.idx[a] = 1.0 / dx[a];
+    }
+    if (out == prim || out == metric || out == K) return fail(GRX_ERR_INVALID_ARG, "out must not alias an input");
+    if (workspace_bytes < (size_t)6 * (size_t)p.nc * (size_t)p.nbox * sizeof(double))
+        return fail(GRX_ERR_INVALID_ARG, "workspace too small");
+    p.prim = prim; p.met = metric; p.K = K; p.out = out;
+    p.gamma = gamma;
+    p.nfallback = t_fallback_counter;
+    p.fb = static_cast<double*>(workspace);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    // The TMA kernel writes the face fluxes of the interior grid lines while it evaluates the right-hand side (p.fb set);
+    // the other kernels do not, and then every face is evaluated by the face kernel.  Same kernel choice as
+    // grx_valencia_rhs, so that out[0..4] are its bits.
+    const int kernel = choose_kernel(p, recon);
+    if (kernel < 0) return fail(GRX_ERR_UNSUPPORTED, "GRX_VARIANT_TMA needs even nx + 2 nghost and 16-byte aligned arrays");
+    const bool fused_faces = (kernel == 2);
+    cudaError_t e;
+    if (fused_faces) {
+        e = grx::launch_rhs_tma(p, recon, 7, st);
+    } else {
+        grx::RhsParams q = p;
+        q.fb = nullptr;
+        e = launch_variant(q, recon, st);
+    }
+    p.nfallback = nullptr;   // the faces next to the block are not faces of the right-hand side: not counted
+    if (e == cudaSuccess) e = grx::launch_face_bflux(p, recon, !fused_faces, st);
+    if (e == cudaSuccess) e = grx::launch_flux_ct(p, st);
+    if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_ct launch");
     return GRX_OK;
 }
 

@@ -14,6 +14,7 @@ struct RhsParams {
     const double* K;       // [nbox][6 ][Nz][Ny][Nx]
     double* out;           // [nbox][8 ][Nz][Ny][Nx]
     unsigned long long* nfallback;   // debug counter or nullptr
+    double* fb;            // [nbox][6][Nz][Ny][Nx] face fluxes of calB for constrained transport, or nullptr
     int n[3];              // interior cells
     int N[3];              // cells incl. ghosts
     int g;                 // ghost width

@@ -18,6 +18,11 @@ bool tma_supported(const RhsParams& p);
 cudaError_t launch_rhs_tma(const RhsParams& p, int recon, int ty, cudaStream_t st);
 double tma_tile_efficiency(const RhsParams& p, int sms);
 
+// grx_ct.cu: NEXT-2, flux-CT of calB.  launch_face_bflux fills p.fb on the lines next to the block (all = every face);
+// launch_flux_ct replaces out[5..7] by the curl of the edge EMFs.
+cudaError_t launch_face_bflux(const RhsParams& p, int recon, bool all, cudaStream_t st);
+cudaError_t launch_flux_ct(const RhsParams& p, cudaStream_t st);
+
 // grx_support.cu
 cudaError_t launch_prim2con(const double* prim, const double* met, long long nc, int nbox, double gamma, double* cons,
                             cudaStream_t st);

@@ -130,7 +130,10 @@ __device__ __forceinline__ void dmetric_smem(const double* mb, double d[10]) {
     for (int f = 0; f < 10; ++f) d[f] = d4raw(mb[f * MF - 2 * S], mb[f * MF - S], mb[f * MF + S], mb[f * MF + 2 * S]);
 }
 
-template <int RECON, int TY>
+// CT: the kernel also writes the HLLE fluxes of the transverse calB components of every face it evaluates to p.fb
+// (constrained transport, grx_valencia_rhs_ct): [6][cell] = F^x(B^y), F^x(B^z), F^y(B^x), F^y(B^z), F^z(B^x), F^z(B^y)
+// at the LOW face of the cell, unscaled.
+template <int RECON, int TY, bool CT>
 __global__ void __launch_bounds__((TY + 1) * 32, 1)
 rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __grid_constant__ CUtensorMap tmP,
                 const __grid_constant__ CUtensorMap tmM, const __grid_constant__ CUtensorMap tmK) {
@@ -160,6 +163,7 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
     const double* __restrict__ met = p.met + (long long)box * 10 * p.nc;
     const double* __restrict__ Kf = p.K + (long long)box * 6 * p.nc;
     double* __restrict__ out = p.out + (long long)box * 8 * p.nc;
+    double* __restrict__ fb = CT ? p.fb + (long long)box * 6 * p.nc : nullptr;
     const long long nc = p.nc, sy = p.stride[1], sz = p.stride[2];
     const double gamma = p.gamma;
     const long long cbase = (X0 + p.g) + sy * (Y0 + p.g) + sz * (k0 - 1 + p.g);   // tile origin, plane k0-1
@@ -279,6 +283,7 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
                         for (int g6 = 0; g6 < 6; ++g6) m.g[g6] = 0.5 * (m1[(4 + g6) * NT] + m0[(4 + g6) * NT]);
                     }
                     face_flux<2>(m, qpz, qm, prim + c - sz, prim + c, nc, gamma, Fh, (kk == 0 && k0 > 0) ? dup : nfb);
+                    if (CT) { fb[4 * nc + c] = Fh[5]; fb[5 * nc + c] = Fh[6]; }
                     // F/dz is rounded once and used with both signs, so a uniform state cancels exactly
 #pragma unroll
                     for (int q = 0; q < 8; ++q) Fh[q] = __dmul_rn(Fh[q], p.idx[2]);
@@ -327,6 +332,7 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
                 FaceGeom m;
                 face_geom_smem<MF, 1>(msb, m);
                 face_flux<0>(m, qx, qm, prim + c - 1, prim + c, nc, gamma, Fx, nfb);
+                if (CT) { fb[c] = Fx[6]; fb[nc + c] = Fx[7]; }
             }
 #pragma unroll
             for (int q = 0; q < 8; ++q) qx[q] = __shfl_down_sync(FULL, Fx[q], 1);   // flux of the high face
@@ -390,6 +396,7 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
                 FaceGeom m;
                 face_geom_smem<MF, MW>(msb, m);
                 face_flux<1>(m, PL, qm, prim + c - sy, prim + c, nc, gamma, Fh, nfb);
+                if (CT) { fb[2 * nc + c] = Fh[5]; fb[3 * nc + c] = Fh[7]; }
 #pragma unroll
                 for (int q = 0; q < 8; ++q) qf[q * EF] = Fh[q];
                 issue_loads(kk + 1, c + sz);
@@ -455,6 +462,7 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
                     face_geom_smem<MF, 1>(mx, m);
                     const long long cxr = cp + sy * xrow + xcol + 1;
                     face_flux<0>(m, PL, PR, prim + cxr - 1, prim + cxr, nc, gamma, Fh, count_x ? nfb : dup);
+                    if (CT) { fb[cxr] = Fh[6]; fb[nc + cxr] = Fh[7]; }
 #pragma unroll
                     for (int q = 0; q < 8; ++q) fxo[q * TY] = Fh[q];
                 }
@@ -478,6 +486,7 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
                 face_geom_smem<MF, MW>(myt, m);
                 const long long cyt = cp + lane + sy * tye;
                 face_flux<1>(m, PL, yt_qm, prim + cyt - sy, prim + cyt, nc, gamma, Fh, count_y ? nfb : dup);
+                if (CT) { fb[2 * nc + cyt] = Fh[5]; fb[3 * nc + cyt] = Fh[7]; }
 #pragma unroll
                 for (int q = 0; q < 8; ++q) QF[q * EF + tye * 32 + lane] = Fh[q];
             }
@@ -551,7 +560,7 @@ TmaGeom make_tiles(const RhsParams& p, int ty, int slots, double* eff_out = null
     return tg;
 }
 
-template <int RECON, int TY>
+template <int RECON, int TY, bool CT>
 cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
     using L = Lay<RECON, TY>;
     int dev = 0, sms = 0;
@@ -566,18 +575,18 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
     const size_t smem = (size_t)L::total * sizeof(double);
     // per device and cheap: set on every launch (no cached state, safe with several devices and host threads)
     // per device and cheap: set on every launch (no cached state, safe with several devices and host threads)
-    e = cudaFuncSetAttribute(rhs_tma_kernel<RECON, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    e = cudaFuncSetAttribute(rhs_tma_kernel<RECON, TY, CT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const TmaGeom tg = make_tiles(p, TY, sms);
     const dim3 grid((unsigned)(tg.ntx * tg.nty * tg.nzc), p.nbox);
-    rhs_tma_kernel<RECON, TY><<<grid, (TY + 1) * 32, smem, st>>>(p, tg, tmP, tmM, tmK);
+    rhs_tma_kernel<RECON, TY, CT><<<grid, (TY + 1) * 32, smem, st>>>(p, tg, tmP, tmM, tmK);
     return cudaGetLastError();
 }
 
 template <int RECON>
 cudaError_t dispatch(const RhsParams& p, int ty, cudaStream_t st) {
     // 7 rows: 8 warps per SM at 254 registers, 211 KB of shared memory (the largest tile whose rings fit)
-    if (ty == 7) return launch_one<RECON, 7>(p, st);
+    if (ty == 7) return p.fb ? launch_one<RECON, 7, true>(p, st) : launch_one<RECON, 7, false>(p, st);
     return cudaErrorInvalidConfiguration;
 }
 

@@ -18,7 +18,7 @@ RECON = {"minmod": 0, "mc": 1, "weno5": 2}
 VARIANT = {"auto": 0, "simple": 1, "ldg": 2, "tma": 3}
 EXPORTS = (
     "grx_valencia_rhs", "grx_valencia_rhs_host", "grx_host_workspace_bytes", "grx_prim2con", "grx_con2prim", "grx_rk_axpy",
-    "grx_step_rk", "grx_step_workspace_bytes", "grx_debug_set_fallback_counter",
+    "grx_step_rk", "grx_step_workspace_bytes", "grx_valencia_rhs_ct", "grx_ct_workspace_bytes", "grx_debug_set_fallback_counter",
     "grx_set_variant", "grx_selftest_math", "grx_dfma_peak_launch", "grx_fp64_issue_probe", "grx_last_error", "grx_version",
     "grx_weno_eps", "grx_v2max",
 )
@@ -54,6 +54,8 @@ def lib():
         L.grx_rk_axpy.argtypes = [gp, i, dbl, vp, dbl, dbl, vp, vp, vp]
         L.grx_step_workspace_bytes.argtypes = [gp, i, i]
         L.grx_step_rk.argtypes = [gp, vp, vp, vp, vp, d3, i, i, dbl, dbl, i, i, i, vp, sz, vp, vp]
+        L.grx_ct_workspace_bytes.argtypes = [gp, i]
+        L.grx_valencia_rhs_ct.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, vp, sz, vp]
         L.grx_debug_set_fallback_counter.argtypes = [vp]
         L.grx_set_variant.argtypes = [i]
         L.grx_selftest_math.argtypes = [vp, vp, sz, vp]
@@ -63,6 +65,7 @@ def lib():
             getattr(L, name).restype = C.c_int
         L.grx_host_workspace_bytes.restype = sz
         L.grx_step_workspace_bytes.restype = sz
+        L.grx_ct_workspace_bytes.restype = sz
         L.grx_last_error.restype = C.c_char_p
         L.grx_weno_eps.restype = dbl
         L.grx_v2max.restype = dbl
@@ -110,6 +113,33 @@ def valencia_rhs(prim, metric, K, dx, nghost, recon, gamma, out=None, stream=Non
     _check(lib().grx_valencia_rhs(C.byref(g), _dev(prim, 8), _dev(metric, 10), _dev(K, 6), dxa, int(nghost), r,
                                   float(gamma), _dev(out, 8), _stream(stream)))
     return out
+
+
+def ct_workspace_bytes(shape, nghost):
+    nbox, _, Nz, Ny, Nx = shape
+    g = grx_grid(Nx - 2 * nghost, Ny - 2 * nghost, Nz - 2 * nghost, nbox)
+    return lib().grx_ct_workspace_bytes(C.byref(g), int(nghost))
+
+
+def valencia_rhs_ct(prim, metric, K, dx, nghost, recon, gamma, out=None, workspace=None, stream=None):
+    """grx_valencia_rhs_ct (NEXT-2): the right-hand side with d calB^i/dt by flux-CT.  `workspace`: CUDA float64 tensor of
+    at least ct_workspace_bytes(prim.shape, nghost) bytes (allocated if not given); on return it holds the six face-flux
+    arrays [nbox, 6, Nz, Ny, Nx].  Returns (out, workspace)."""
+    import torch
+    if out is None:
+        out = torch.empty_like(prim)
+    if workspace is None:
+        workspace = torch.empty((prim.shape[0], 6) + tuple(prim.shape[2:]), dtype=torch.float64, device=prim.device)
+    g = _grid(prim, nghost)
+    if metric.shape[0] != prim.shape[0] or K.shape[0] != prim.shape[0] or metric.shape[2:] != prim.shape[2:] \
+            or K.shape[2:] != prim.shape[2:] or out.shape != prim.shape:
+        raise GrxError("prim, metric, K, out must share nbox and the spatial shape")
+    r = RECON[recon] if isinstance(recon, str) else int(recon)
+    dxa = (C.c_double * 3)(*[float(v) for v in dx])
+    _check(lib().grx_valencia_rhs_ct(C.byref(g), _dev(prim, 8), _dev(metric, 10), _dev(K, 6), dxa, int(nghost), r,
+                                     float(gamma), _dev(out, 8), C.c_void_p(workspace.data_ptr()),
+                                     workspace.numel() * workspace.element_size(), _stream(stream)))
+    return out, workspace
 
 
 def host_workspace_bytes(shape, nghost):
