@@ -326,6 +326,41 @@ def time_ct(grx, torch, prob, dev, recon, stream, steps=10):
             "scheme": f"flux-CT of calB (reading R30), {recon}+HLLE; {prob.name}"}
 
 
+def time_halo_overlap(grx, torch, prob, dev, recon, stream, world, nsteps=3):
+    """NEXT-4: SSP-RK2 steps of a z-slab ring (this rank's block = one slab; periodic in x, y per rank and in z over the
+    ring of ranks; a single rank is its own neighbour) with the ghost exchange overlapped with the interior planes
+    (paper_2210_17509_b200/halo.py) and, for comparison, exchanged first."""
+    from paper_2210_17509_b200 import halo
+    prim0, met, K = dev
+    g = prob.nghost
+    res = {}
+    for overlap in (True, False):
+        prim = prim0.clone()
+        grx.fill_ghosts(prim, g, "periodic", 7, stream=stream)
+        cons = grx.prim2con(prim, met, g, prob.gamma)
+        ex = halo.ZSlabExchange(prim, g)
+        work = (torch.empty_like(cons), torch.empty_like(cons))
+        dt = 0.2 * min(prob.dx)
+        halo.step_rk2_zslabs(ex, cons, prim, met, K, prob.dx, g, recon, prob.gamma, dt, 1, work, overlap=overlap, stream=stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        halo.step_rk2_zslabs(ex, cons, prim, met, K, prob.dx, g, recon, prob.gamma, dt, nsteps, work, overlap=overlap,
+                             stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        t = max_over_ranks(e0.elapsed_time(e1) * 1e-3, world, "cuda")
+        res["overlapped" if overlap else "exchange_first"] = {"zone_cycles_per_s": prob.cells * world * nsteps / t,
+                                                              "ms_per_step": 1e3 * t / nsteps}
+        res["finite"] = bool(torch.isfinite(cons[prob.interior]).all().item())
+        res["bytes_per_exchange_per_rank"] = ex.bytes_per_exchange
+        del ex, work, cons, prim
+    res["ranks"] = world
+    res["scheme"] = (f"z-slab ring of {world} rank(s), one {prob.name} block each, SSP-RK2, {recon}+HLLE, periodic; "
+                     "2 exchanges of 2 x 3 ghost planes x 8 fields per step")
+    return res
+
+
 def measure_dfma_peak(grx, torch, stream):
     sink = torch.zeros(1, dtype=torch.float64, device="cuda")
     grx.dfma_peak_launch(2000, sink, stream)
@@ -435,6 +470,12 @@ def run_ours(args):
     d2h = int(ho.numel() * 8)
     del ws, hp, hm, hk, ho
 
+    # ---- NEXT-4: z-slab ring with the ghost exchange overlapped (every rank takes part; with more than one rank only on
+    # request, as the point-to-point path has been exercised on CPU ranks only)
+    halo_res = None
+    if (world == 1 and not args.no_sweep and prob.nbox == 1) or args.halo:
+        halo_res = time_halo_overlap(grx, torch, prob, dev, recon, stream, world)
+
     if rank != 0:
         if world > 1:
             dist.barrier()
@@ -515,6 +556,8 @@ def run_ours(args):
         line["zone_cycles"] = zone_cycles
     if ct is not None:
         line["constrained_transport"] = ct
+    if halo_res is not None:
+        line["halo_overlap"] = halo_res
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()
@@ -578,6 +621,8 @@ def main():
                     help="kernel selector (auto = product path)")
     ap.add_argument("--no-sweep", action="store_true", help="leave the config sweep out of the contract line")
     ap.add_argument("--sweep", action="store_true", help="time every config instead of the contract line")
+    ap.add_argument("--halo", action="store_true", help="also time the z-slab ring with overlapped ghost exchange (NEXT-4) "
+                                                        "when there is more than one rank")
     args = ap.parse_args()
     if args.steps < 1:
         raise SystemExit("--steps must be >= 1")

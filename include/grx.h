@@ -159,6 +159,31 @@ int grx_valencia_rhs_ct(const grx_grid* grid, const double* prim, const double* 
                         const double dx[3], int nghost, int recon, double gamma, double* out, void* workspace,
                         size_t workspace_bytes, void* cuda_stream);
 
+/* NEXT-4 (PAPER.md l.222-230 ghost-zone fill between blocks, l.371 "start the computations of those
+ * cells ... which do not need ghost cells while ghost cells ... are getting filled, and then compute the remaining cells
+ * thereafter"): the pieces a slab decomposition along z needs to overlap the ghost exchange with the interior update.
+ * paper_2210_17509_b200/halo.py composes them with torch.distributed point-to-point transfers.
+ *
+ * grx_valencia_rhs_zrange: the right-hand side on the interior planes k_begin <= k < k_end only (nbox = 1); every plane gets
+ *   the bits of the whole-block call (same kernel choice, same arithmetic per cell).  Planes g <= k < nz - g read no z ghost
+ *   plane and can run while those are in flight; [0, g) and [nz - g, nz) follow when they have arrived.
+ * grx_halo_z: pack (unpack = 0) the nghost lowest (side 0) or highest (side 1) INTERIOR planes of the 8 primitive fields into
+ *   buf[nbox][8][nghost][Ny][Nx], or unpack (unpack = 1) buf into the low (side 0) / high (side 1) z GHOST planes.  Planes
+ *   travel with their x and y ghost cells (fill those first).  buf: DEVICE, grx_halo_z_bytes(grid, nghost) bytes.
+ * grx_fill_ghosts: the ghost fill of grx_step_rk as a call of its own; dirs = mask of the directions filled here (bit 0 = x,
+ *   1 = y, 2 = z): a z-slab rank fills x and y (dirs = 3) and receives z.
+ * grx_rk_stage: the stage update of grx_step_rk as a call of its own: Uout = a Ua + b (Ub + h L) on the interior cells,
+ *   acc += wdt L if acc is non-NULL, prim = con2prim(Uout) (Gamma-law, R22); nfail as for grx_con2prim. */
+int grx_valencia_rhs_zrange(const grx_grid* grid, const double* prim, const double* metric, const double* K,
+                            const double dx[3], int nghost, int recon, double gamma, double* out, int k_begin, int k_end,
+                            void* cuda_stream);
+size_t grx_halo_z_bytes(const grx_grid* grid, int nghost);
+int grx_halo_z(const grx_grid* grid, double* prim, int nghost, int side, int unpack, double* buf, void* cuda_stream);
+int grx_fill_ghosts(const grx_grid* grid, double* prim, int nghost, int bc, int dirs, void* cuda_stream);
+int grx_rk_stage(const grx_grid* grid, int nghost, double a, const double* Ua, double b, const double* Ub, double h,
+                 const double* L, double* Uout, double* acc, double wdt, const double* metric, double gamma, double* prim,
+                 unsigned long long* nfail, void* cuda_stream);
+
 /* Debug: if `counter` (DEVICE pointer to one unsigned long long, caller-zeroed) is non-NULL, later
  * grx_valencia_rhs calls of this host thread add to it the number of face sides that took the R5
  * first-order fallback.  NULL switches counting off (the default; counting costs a few atomics). */

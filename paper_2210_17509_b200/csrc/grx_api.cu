@@ -291,6 +291,94 @@ int grx_rk_axpy(const grx_grid* grid, int nghost, double a, const double* x, dou
     return GRX_OK;
 }
 
+int grx_valencia_rhs_zrange(const grx_grid* grid, const double* prim, const double* metric, const double* K,
+                            const double dx[3], int nghost, int recon, double gamma, double* out, int k_begin, int k_end,
+                            void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim || !metric || !K || !dx || !out) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (recon != GRX_RECON_MINMOD && recon != GRX_RECON_MC && recon != GRX_RECON_WENO5)
+        return fail(GRX_ERR_INVALID_ARG, "unknown recon");
+    if (nghost < (recon == GRX_RECON_WENO5 ? 3 : 2))
+        return fail(GRX_ERR_INVALID_ARG, "nghost too small: WENO5 needs 3, minmod/MC need 2 (R29)");
+    if (!(gamma > 1.0)) return fail(GRX_ERR_INVALID_ARG, "gamma must be > 1");
+    for (int a = 0; a < 3; ++a) {
+        if (!(dx[a] > 0.0) || !(1.0 / dx[a] > 0.0)) return fail(GRX_ERR_INVALID_ARG, "dx must be > 0 and finite");
+        p.idx[a] = 1.0 / dx[a];
+    }
+    if (out == prim || out == metric || out == K) return fail(GRX_ERR_INVALID_ARG, "out must not alias an input");
+    if (k_begin < 0 || k_end > p.n[2] || k_begin > k_end) return fail(GRX_ERR_INVALID_ARG, "need 0 <= k_begin <= k_end <= nz");
+    if (p.nbox != 1 && !(k_begin == 0 && k_end == p.n[2]))
+        return fail(GRX_ERR_INVALID_ARG, "a z range of a batch is not contiguous: nbox must be 1");
+    if (k_begin == k_end) return GRX_OK;
+    p.prim = prim; p.met = metric; p.K = K; p.out = out;
+    p.gamma = gamma;
+    p.nfallback = t_fallback_counter;
+    // the kernel the whole block would get, so that the planes carry the bits of the whole-block call
+    const int kernel = choose_kernel(p, recon);
+    if (kernel < 0) return fail(GRX_ERR_UNSUPPORTED, "GRX_VARIANT_TMA needs even nx + 2 nghost and 16-byte aligned arrays");
+    // the sub-block of planes [k_begin, k_end): same arrays, shifted by k_begin planes, nz = k_end - k_begin; the field
+    // stride nc stays that of the whole block
+    const int nz_whole = p.n[2];
+    const size_t off = (size_t)k_begin * (size_t)p.stride[2];
+    p.prim += off; p.met += off; p.K += off; p.out += off;
+    p.n[2] = k_end - k_begin;
+    p.N[2] = p.n[2] + 2 * p.g;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    cudaError_t e = kernel == 0 ? grx::launch_rhs_simple(p, recon, st)
+                  : kernel == 1 ? grx::launch_rhs_fused(p, recon, st, nz_whole) : grx::launch_rhs_tma(p, recon, 7, st);
+    if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_zrange launch");
+    return GRX_OK;
+}
+
+int grx_rk_stage(const grx_grid* grid, int nghost, double a, const double* Ua, double b, const double* Ub, double h,
+                 const double* L, double* Uout, double* acc, double wdt, const double* metric, double gamma, double* prim,
+                 unsigned long long* nfail, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!Ua || !Ub || !L || !Uout || !metric || !prim) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (!(gamma > 1.0)) return fail(GRX_ERR_INVALID_ARG, "gamma must be > 1");
+    p.met = metric;
+    p.gamma = gamma;
+    const cudaError_t e = grx::launch_rk_stage(p, a, Ua, b, Ub, h, L, Uout, acc, wdt, prim, nfail,
+                                               static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_rk_stage launch");
+    return GRX_OK;
+}
+
+int grx_fill_ghosts(const grx_grid* grid, double* prim, int nghost, int bc, int dirs, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (bc != GRX_BC_COPY && bc != GRX_BC_PERIODIC) return fail(GRX_ERR_INVALID_ARG, "unknown boundary condition");
+    if (dirs < 0 || dirs > 7) return fail(GRX_ERR_INVALID_ARG, "dirs is a mask of bits 0..2");
+    const cudaError_t e = grx::launch_fill_ghosts(p, prim, bc, dirs, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_fill_ghosts launch");
+    return GRX_OK;
+}
+
+size_t grx_halo_z_bytes(const grx_grid* grid, int nghost) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (make_geom(grid, nghost, p)) return 0;
+    return (size_t)p.nbox * 8 * (size_t)p.g * (size_t)p.stride[2] * sizeof(double);
+}
+
+int grx_halo_z(const grx_grid* grid, double* prim, int nghost, int side, int unpack, double* buf, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim || !buf) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (side != 0 && side != 1) return fail(GRX_ERR_INVALID_ARG, "side must be 0 (low) or 1 (high)");
+    if (p.n[2] < p.g) return fail(GRX_ERR_INVALID_ARG, "a slab must have at least nghost planes");
+    const cudaError_t e = grx::launch_halo_z(p, prim, buf, side, unpack != 0, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_halo_z launch");
+    return GRX_OK;
+}
+
 size_t grx_ct_workspace_bytes(const grx_grid* grid, int nghost) {
     grx::RhsParams p;
     std::memset(&p, 0, sizeof(p));
@@ -383,7 +471,7 @@ int grx_step_rk(const grx_grid* grid, double* cons, double* prim, const double* 
     auto rhs = [&]() { return launch_variant(p, recon, st); };
     auto stage = [&](double a, const double* Ua, double b, const double* Ub, double h, double* ac, double wdt) {
         cudaError_t r = grx::launch_rk_stage(p, a, Ua, b, Ub, h, L, cons, ac, wdt, prim, nfail, st);
-        return r != cudaSuccess ? r : grx::launch_fill_ghosts(p, prim, bc, st);
+        return r != cudaSuccess ? r : grx::launch_fill_ghosts(p, prim, bc, 7, st);
     };
     // L lives in the workspace: its ghost cells are never read or written
     for (int s = 0; s < nsteps && e == cudaSuccess; ++s) {

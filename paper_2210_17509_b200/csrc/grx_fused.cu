@@ -311,9 +311,11 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
 
 // 11 rows (12 warps per SM at 168 registers); blocks that are thin along z have too few plane steps per CTA to
 // amortise the taller tile and take the 7-row one (8 warps, 255 registers).
+// tile_nz: the plane count the tile is chosen for -- that of the whole block when p is a z range of it, so that every
+// plane carries the bits of the whole-block call (the two instantiations round differently).
 template <int RECON>
-cudaError_t dispatch(const RhsParams& p, cudaStream_t st) {
-    if (p.n[2] < 8) return launch_one<RECON, 7, 1>(p, st);
+cudaError_t dispatch(const RhsParams& p, int tile_nz, cudaStream_t st) {
+    if (tile_nz < 8) return launch_one<RECON, 7, 1>(p, st);
     return launch_one<RECON, 11, 1>(p, st);
 }
 
@@ -325,10 +327,11 @@ double fused_tile_efficiency(const RhsParams& p, int sms) {
     return eff;
 }
 
-cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st) {
-    if (recon == RECON_WENO5) return dispatch<RECON_WENO5>(p, st);
-    if (recon == RECON_MC) return dispatch<RECON_MC>(p, st);
-    return dispatch<RECON_MINMOD>(p, st);
+cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st, int tile_nz) {
+    if (tile_nz <= 0) tile_nz = p.n[2];
+    if (recon == RECON_WENO5) return dispatch<RECON_WENO5>(p, tile_nz, st);
+    if (recon == RECON_MC) return dispatch<RECON_MC>(p, tile_nz, st);
+    return dispatch<RECON_MINMOD>(p, tile_nz, st);
 }
 
 }  // namespace grx

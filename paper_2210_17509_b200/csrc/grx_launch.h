@@ -10,7 +10,7 @@ namespace grx {
 // grx_simple.cu: one thread per cell, every thread evaluates its own six faces (cross-check variant)
 cudaError_t launch_rhs_simple(const RhsParams& p, int recon, cudaStream_t st);
 // grx_fused.cu: the round-1 kernel (operands through L1), the path for arrays the TMA kernel cannot take
-cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st);
+cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st, int tile_nz = 0);   // tile_nz: see grx_fused.cu
 double fused_tile_efficiency(const RhsParams& p, int sms);   // expected fill of the launch geometry, in (0, 1]
 
 // grx_tma.cu: the product kernel (TMA-staged planes, shared-memory z rings); needs even Nx and 16-byte aligned arrays
@@ -33,7 +33,8 @@ cudaError_t launch_rk_axpy(const RhsParams& geom, double a, const double* x, dou
 cudaError_t launch_rk_stage(const RhsParams& geom, double a, const double* Ua, double b, const double* Ub, double h,
                             const double* L, double* Uout, double* acc, double wdt, double* prim, unsigned long long* nfail,
                             cudaStream_t st);
-cudaError_t launch_fill_ghosts(const RhsParams& geom, double* prim, int bc, cudaStream_t st);
+cudaError_t launch_fill_ghosts(const RhsParams& geom, double* prim, int bc, int dirs, cudaStream_t st);
+cudaError_t launch_halo_z(const RhsParams& geom, double* prim, double* buf, int side, bool unpack, cudaStream_t st);
 cudaError_t launch_selftest_math(const double* x, double* y, size_t n, cudaStream_t st);
 cudaError_t launch_dfma_peak(int iters, double* sink, double* flops_out, cudaStream_t st);
 cudaError_t launch_issue_probe(int mode, int iters, double* sink, double* fp64_instr_out, cudaStream_t st);

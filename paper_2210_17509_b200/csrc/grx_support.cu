@@ -91,7 +91,9 @@ __global__ void __launch_bounds__(128) rk_stage_kernel(const __grid_constant__ R
 
 // NEXT-1: ghost fill of the 8 primitives at the outer boundary of every box (l.170, l.255, l.329): a ghost cell takes the
 // interior cell whose index is its own, clamped (bc = 0, "copy") or wrapped (bc = 1, periodic) direction by direction.
-__global__ void __launch_bounds__(256) fill_ghosts_kernel(const __grid_constant__ RhsParams p, double* prim, int bc) {
+// `dirs`: bit d set = direction d is filled here; a cell that is a ghost cell only in other directions is left alone
+// (NEXT-4: the z ghost planes of a slab decomposition come from the neighbour ranks).
+__global__ void __launch_bounds__(256) fill_ghosts_kernel(const __grid_constant__ RhsParams p, double* prim, int bc, int dirs) {
     const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= p.nc) return;
     const int I = (int)(c % p.N[0]), J = (int)((c / p.N[0]) % p.N[1]), Kz = (int)(c / p.stride[2]);
@@ -101,17 +103,35 @@ __global__ void __launch_bounds__(256) fill_ghosts_kernel(const __grid_constant_
     for (int d = 0; d < 3; ++d) {
         const int n = p.n[d];
         int v = s[d];
-        if (v < 0 || v >= n) {
+        if ((v < 0 || v >= n) && ((dirs >> d) & 1)) {
             ghost = true;
             v = bc == 1 ? ((v % n) + n) % n : (v < 0 ? 0 : n - 1);
         }
         s[d] = v;
     }
     if (!ghost) return;
+    // unfilled directions keep their own (ghost) index: s[d] + g is the cell's own coordinate there
     const long long src = (s[0] + p.g) + p.stride[1] * (s[1] + p.g) + p.stride[2] * (s[2] + p.g);
     double* pb = prim + (long long)blockIdx.y * 8 * p.nc;
 #pragma unroll
     for (int q = 0; q < 8; ++q) pb[q * p.nc + c] = pb[q * p.nc + src];
+}
+
+
+// NEXT-4: the z ghost planes of a slab decomposition.  side 0: the g lowest
+// interior planes (sent to the rank below, whose high ghost planes they fill), side 1: the g highest interior planes.
+// buf[box][field][g][Ny][Nx], planes complete with their x and y ghost cells (fill those first: corners come along).
+// unpack: side 0 = the g low ghost planes, side 1 = the g high ghost planes.
+__global__ void __launch_bounds__(256) halo_z_kernel(const __grid_constant__ RhsParams p, double* prim, double* buf, int side,
+                                                     int unpack) {
+    const long long slab = (long long)p.g * p.stride[2];
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= slab) return;
+    const int bf = blockIdx.y;   // box * 8 + field
+    const int k0 = unpack ? (side == 0 ? 0 : p.n[2] + p.g) : (side == 0 ? p.g : p.n[2]);
+    double* a = prim + (long long)bf * p.nc + (long long)k0 * p.stride[2] + t;
+    double* b = buf + (long long)bf * slab + t;
+    if (unpack) *a = *b; else *b = *a;
 }
 
 __global__ void selftest_math_kernel(const double* __restrict__ x, double* __restrict__ y, size_t n) {
@@ -173,9 +193,17 @@ cudaError_t launch_rk_stage(const RhsParams& p, double a, const double* Ua, doub
     return cudaGetLastError();
 }
 
-cudaError_t launch_fill_ghosts(const RhsParams& p, double* prim, int bc, cudaStream_t st) {
+cudaError_t launch_fill_ghosts(const RhsParams& p, double* prim, int bc, int dirs, cudaStream_t st) {
     const dim3 grid((unsigned)((p.nc + 255) / 256), p.nbox);
-    fill_ghosts_kernel<<<grid, 256, 0, st>>>(p, prim, bc);
+    fill_ghosts_kernel<<<grid, 256, 0, st>>>(p, prim, bc, dirs);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_halo_z(const RhsParams& p, double* prim, double* buf, int side, bool unpack, cudaStream_t st) {
+    const long long slab = (long long)p.g * p.stride[2];
+    if (slab == 0) return cudaSuccess;
+    const dim3 grid((unsigned)((slab + 255) / 256), (unsigned)(p.nbox * 8));
+    halo_z_kernel<<<grid, 256, 0, st>>>(p, prim, buf, side, unpack ? 1 : 0);
     return cudaGetLastError();
 }
 

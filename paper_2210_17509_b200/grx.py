@@ -18,7 +18,8 @@ RECON = {"minmod": 0, "mc": 1, "weno5": 2}
 VARIANT = {"auto": 0, "simple": 1, "ldg": 2, "tma": 3}
 EXPORTS = (
     "grx_valencia_rhs", "grx_valencia_rhs_host", "grx_host_workspace_bytes", "grx_prim2con", "grx_con2prim", "grx_rk_axpy",
-    "grx_step_rk", "grx_step_workspace_bytes", "grx_valencia_rhs_ct", "grx_ct_workspace_bytes", "grx_debug_set_fallback_counter",
+    "grx_step_rk", "grx_step_workspace_bytes", "grx_valencia_rhs_ct", "grx_ct_workspace_bytes",
+    "grx_valencia_rhs_zrange", "grx_halo_z", "grx_halo_z_bytes", "grx_fill_ghosts", "grx_rk_stage", "grx_debug_set_fallback_counter",
     "grx_set_variant", "grx_selftest_math", "grx_dfma_peak_launch", "grx_fp64_issue_probe", "grx_last_error", "grx_version",
     "grx_weno_eps", "grx_v2max",
 )
@@ -56,6 +57,11 @@ def lib():
         L.grx_step_rk.argtypes = [gp, vp, vp, vp, vp, d3, i, i, dbl, dbl, i, i, i, vp, sz, vp, vp]
         L.grx_ct_workspace_bytes.argtypes = [gp, i]
         L.grx_valencia_rhs_ct.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, vp, sz, vp]
+        L.grx_valencia_rhs_zrange.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, i, i, vp]
+        L.grx_halo_z_bytes.argtypes = [gp, i]
+        L.grx_halo_z.argtypes = [gp, vp, i, i, i, vp, vp]
+        L.grx_fill_ghosts.argtypes = [gp, vp, i, i, i, vp]
+        L.grx_rk_stage.argtypes = [gp, i, dbl, vp, dbl, vp, dbl, vp, vp, vp, dbl, vp, dbl, vp, vp, vp]
         L.grx_debug_set_fallback_counter.argtypes = [vp]
         L.grx_set_variant.argtypes = [i]
         L.grx_selftest_math.argtypes = [vp, vp, sz, vp]
@@ -66,6 +72,7 @@ def lib():
         L.grx_host_workspace_bytes.restype = sz
         L.grx_step_workspace_bytes.restype = sz
         L.grx_ct_workspace_bytes.restype = sz
+        L.grx_halo_z_bytes.restype = sz
         L.grx_last_error.restype = C.c_char_p
         L.grx_weno_eps.restype = dbl
         L.grx_v2max.restype = dbl
@@ -224,6 +231,46 @@ def step_rk(cons, prim, metric, K, dx, nghost, recon, gamma, dt, nsteps, rk=2, b
                              C.c_void_p(workspace.data_ptr()), workspace.numel() * workspace.element_size(), nf,
                              _stream(stream)))
     return cons, prim
+
+
+def valencia_rhs_zrange(prim, metric, K, dx, nghost, recon, gamma, out, k_begin, k_end, stream=None):
+    """grx_valencia_rhs_zrange (NEXT-4): the right-hand side on the interior planes k_begin <= k < k_end of a single box."""
+    g = _grid(prim, nghost)
+    r = RECON[recon] if isinstance(recon, str) else int(recon)
+    dxa = (C.c_double * 3)(*[float(v) for v in dx])
+    _check(lib().grx_valencia_rhs_zrange(C.byref(g), _dev(prim, 8), _dev(metric, 10), _dev(K, 6), dxa, int(nghost), r,
+                                         float(gamma), _dev(out, 8), int(k_begin), int(k_end), _stream(stream)))
+    return out
+
+
+def halo_z_bytes(shape, nghost):
+    nbox, _, Nz, Ny, Nx = shape
+    g = grx_grid(Nx - 2 * nghost, Ny - 2 * nghost, Nz - 2 * nghost, nbox)
+    return lib().grx_halo_z_bytes(C.byref(g), int(nghost))
+
+
+def halo_z(prim, nghost, side, unpack, buf, stream=None):
+    """grx_halo_z (NEXT-4): pack the nghost lowest / highest interior planes of prim into buf, or unpack buf into the low /
+    high z ghost planes."""
+    g = _grid(prim, nghost)
+    _check(lib().grx_halo_z(C.byref(g), _dev(prim, 8), int(nghost), int(side), int(bool(unpack)),
+                            C.c_void_p(buf.data_ptr()), _stream(stream)))
+
+
+def fill_ghosts(prim, nghost, bc="periodic", dirs=7, stream=None):
+    g = _grid(prim, nghost)
+    _check(lib().grx_fill_ghosts(C.byref(g), _dev(prim, 8), int(nghost), BC[bc] if isinstance(bc, str) else int(bc),
+                                 int(dirs), _stream(stream)))
+
+
+def rk_stage(nghost, a, Ua, b, Ub, h, L, Uout, metric, gamma, prim, acc=None, wdt=0.0, nfail=None, stream=None):
+    """grx_rk_stage: Uout = a Ua + b (Ub + h L) on the interior, acc += wdt L, prim = con2prim(Uout)."""
+    g = _grid(prim, nghost)
+    nul = C.c_void_p(0)
+    _check(lib().grx_rk_stage(C.byref(g), int(nghost), float(a), _dev(Ua, 8), float(b), _dev(Ub, 8), float(h), _dev(L, 8),
+                              _dev(Uout, 8), _dev(acc, 8) if acc is not None else nul, float(wdt), _dev(metric, 10),
+                              float(gamma), _dev(prim, 8), C.c_void_p(nfail.data_ptr()) if nfail is not None else nul,
+                              _stream(stream)))
 
 
 def set_fallback_counter(counter):
