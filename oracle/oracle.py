@@ -54,6 +54,10 @@ def lib():
         L.oracle_face_bfluxes.restype = C.c_int
         L.oracle_flux_ct.argtypes = [ip, C.c_int, dp, dp, C.c_int, dp]
         L.oracle_flux_ct.restype = C.c_int
+        L.oracle_valencia_rhs_vertex.argtypes = [ip, C.c_int, dp, dp, dp, dp, C.c_int, C.c_int, C.c_double, dp, up]
+        L.oracle_valencia_rhs_vertex.restype = C.c_int
+        L.oracle_tmunu_vertices.argtypes = [ip, C.c_int, dp, dp, C.c_int, C.c_double, dp]
+        L.oracle_tmunu_vertices.restype = C.c_int
         L.oracle_weno_eps.restype = C.c_double
         L.oracle_v2max.restype = C.c_double
         _lib = L
@@ -151,6 +155,31 @@ def valencia_rhs_ct(prim, metric, K, dx, nghost, recon, gamma):
     dB = flux_ct(face_bfluxes(prim, metric, nghost, recon, gamma), dx, nghost)
     out[:, 5:8] = dB
     return out, nfb
+
+
+def valencia_rhs_vertex(prim, metric_v, K_v, dx, nghost, recon, gamma):
+    """NEXT-3 (R31): the right-hand side with the metric and K_ij sampled at the cell VERTICES,
+    metric_v[nbox, 10, Nz+1, Ny+1, Nx+1] (vertex (I,J,K) = low corner of cell (I,J,K)).  Returns (out, nfallback)."""
+    prim, metric_v, K_v = _arr(prim), _arr(metric_v), _arr(K_v)
+    n, nbox = _grid(prim, nghost)
+    assert metric_v.shape == (nbox, 10) + tuple(s + 1 for s in prim.shape[2:]) and K_v.shape[1] == 6
+    out = np.full(prim.shape, np.nan)
+    nfb = C.c_ulonglong(0)
+    r = RECON[recon] if isinstance(recon, str) else int(recon)
+    if lib().oracle_valencia_rhs_vertex(n, nbox, _p(prim), _p(metric_v), _p(K_v), (C.c_double * 3)(*dx), nghost, r, gamma,
+                                        _p(out), C.byref(nfb)):
+        raise ValueError("oracle: invalid argument")
+    return out, int(nfb.value)
+
+
+def tmunu_vertices(prim, metric_v, nghost, gamma):
+    """NEXT-3 (R32): T^{mu nu} (10 components) at the vertices of the interior cells; NaN elsewhere."""
+    prim, metric_v = _arr(prim), _arr(metric_v)
+    n, nbox = _grid(prim, nghost)
+    T = np.full((nbox, 10) + metric_v.shape[2:], np.nan)
+    if lib().oracle_tmunu_vertices(n, nbox, _p(prim), _p(metric_v), nghost, gamma, _p(T)):
+        raise ValueError("oracle: invalid argument")
+    return T
 
 
 BC = {"copy": 0, "periodic": 1}

@@ -669,6 +669,197 @@ void flux_ct_box(const Grid& G, const double* FB, const double dx[3], double* dB
             }
 }
 
+// ---- NEXT-3: vertex-centred spacetime, readings R31 / R32 -----------------------------------
+// "Spacetime geometry quantities are stored on vertices", "the spacetime metric ... is known at the cell
+// vertices and is interpolated linearly to the face centers" (l.130), "the stress-energy tensor [is] stored as samples at
+// the cell vertices ... we perform a 4th-order symmetric 3D interpolation from cell center values to calculate the fluid
+// variables at cell vertices" (l.84, l.323).
+// Vertex arrays: [field][Nz+1][Ny+1][Nx+1]; vertex (I, J, K) is the LOW corner of cell (I, J, K) (indices with ghosts), so
+// cell (I, J, K) has the eight vertices (I..I+1, J..J+1, K..K+1) and its low d-face the four with the d index fixed.
+// R31: face metric = arithmetic mean of the 4 vertices of the face (linear interpolation to the face centre); cell-centre
+//      metric and K_ij = mean of the 8 vertices; d_a of a metric field at the cell centre = staggered 4th-order difference
+//      [27 (m(i+1/2) - m(i-1/2)) - (m(i+3/2) - m(i-3/2))] / (24 dx_a) of the transverse 4-vertex means m(.) at the four
+//      vertex planes around the cell, grouped so that a constant differentiates to exactly zero.  Everything else is the
+//      right-hand side of rhs_box.
+struct VGrid {
+    Grid G;
+    size_t nv;                // vertices per field
+    size_t vidx(int i, int j, int k) const {   // vertex at the low corner of the cell with INTERIOR index (i, j, k)
+        return (size_t)(i + G.g) + (size_t)(G.N[0] + 1) * ((size_t)(j + G.g) + (size_t)(G.N[1] + 1) * (size_t)(k + G.g));
+    }
+};
+
+// mean of the 4 vertices of the low d-face of cell (i, j, k)
+inline double face_mean(const VGrid& V, const double* f, int d, int i, int j, int k) {
+    const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+    double sum = 0.0;
+    for (int a = 0; a < 2; ++a)
+        for (int b = 0; b < 2; ++b) {
+            int c[3] = {i, j, k};
+            c[d1] += a;
+            c[d2] += b;
+            sum += f[V.vidx(c[0], c[1], c[2])];
+        }
+    return 0.25 * sum;
+}
+
+void rhs_vertex_box(const VGrid& V, const double* prim, const double* metv, const double* Kv, const double dx[3], int recon,
+                    double gamma, double* out, unsigned long long* fallback_total) {
+    const Grid& G = V.G;
+    const size_t NC = G.ncell, NV = V.nv;
+    unsigned long long nfb_all = 0;
+    for (int c = 0; c < 8; ++c)
+        for (int k = 0; k < G.n[2]; ++k)
+            for (int j = 0; j < G.n[1]; ++j)
+                for (int i = 0; i < G.n[0]; ++i) out[c * NC + G.idx(i, j, k)] = 0.0;
+    for (int d = 0; d < 3; ++d) {
+        const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+        const int nd = G.n[d];
+        const long nlines = (long)G.n[d1] * G.n[d2];
+#pragma omp parallel
+        {
+            unsigned long long nfb = 0;
+            std::vector<double> qm(8 * (size_t)(nd + 2)), qp(8 * (size_t)(nd + 2)), Fh(8 * (size_t)(nd + 1));
+#pragma omp for schedule(static)
+            for (long line = 0; line < nlines; ++line) {
+                int ijk[3];
+                ijk[d1] = (int)(line % G.n[d1]);
+                ijk[d2] = (int)(line / G.n[d1]);
+                auto cell = [&](int s, int c3[3]) { c3[0] = ijk[0]; c3[1] = ijk[1]; c3[2] = ijk[2]; c3[d] = s; };
+                auto at = [&](int s) { int c3[3]; cell(s, c3); return G.idx(c3[0], c3[1], c3[2]); };
+                for (int s = -1; s <= nd; ++s)
+                    for (int q = 0; q < 8; ++q) {
+                        const double* f = prim + q * NC;
+                        const double a = (recon == RECON_WENO5) ? f[at(s - 2)] : 0.0;
+                        const double e = (recon == RECON_WENO5) ? f[at(s + 2)] : 0.0;
+                        recon_cell<double>(recon, a, f[at(s - 1)], f[at(s)], f[at(s + 1)], e, qm[q * (nd + 2) + s + 1],
+                                           qp[q * (nd + 2) + s + 1]);
+                    }
+                for (int f = 0; f <= nd; ++f) {
+                    const size_t iL = at(f - 1), iR = at(f);
+                    int c3[3];
+                    cell(f, c3);                                   // the face is the low d-face of cell f
+                    Metric<double> mf;
+                    mf.alp = face_mean(V, metv + 0 * NV, d, c3[0], c3[1], c3[2]);                       // R31
+                    for (int i = 0; i < 3; ++i) mf.beta[i] = face_mean(V, metv + (1 + i) * NV, d, c3[0], c3[1], c3[2]);
+                    for (int c = 0; c < 6; ++c) mf.g[c] = face_mean(V, metv + (4 + c) * NV, d, c3[0], c3[1], c3[2]);
+                    double PL[8], PR[8], CL[8], CR[8];
+                    for (int q = 0; q < 8; ++q) {
+                        PL[q] = qp[q * (nd + 2) + f];
+                        PR[q] = qm[q * (nd + 2) + f + 1];
+                        CL[q] = prim[q * NC + iL];
+                        CR[q] = prim[q * NC + iR];
+                    }
+                    face_flux(mf, d, gamma, PL, PR, CL, CR, &Fh[8 * (size_t)f], &nfb);
+                }
+                for (int s = 0; s < nd; ++s)
+                    for (int c = 0; c < 8; ++c) out[c * NC + at(s)] -= (Fh[8 * (size_t)(s + 1) + c] - Fh[8 * (size_t)s + c]) / dx[d];
+            }
+#pragma omp critical
+            nfb_all += nfb;
+        }
+    }
+#pragma omp parallel for schedule(static) collapse(2)
+    for (int k = 0; k < G.n[2]; ++k)
+        for (int j = 0; j < G.n[1]; ++j)
+            for (int i = 0; i < G.n[0]; ++i) {
+                const size_t c0 = G.idx(i, j, k);
+                double dm[3][10];
+                Metric<double> mc;
+                double mcv[10], K[6];
+                for (int f = 0; f < 10; ++f) {
+                    const double* mv = metv + f * NV;
+                    // centre = mean of 8 vertices = mean of the low and the high x-face means
+                    mcv[f] = 0.5 * (face_mean(V, mv, 0, i, j, k) + face_mean(V, mv, 0, i + 1, j, k));
+                    for (int a = 0; a < 3; ++a) {
+                        int lo2[3] = {i, j, k}, lo1[3] = {i, j, k}, hi1[3] = {i, j, k}, hi2[3] = {i, j, k};
+                        lo2[a] -= 1; hi1[a] += 1; hi2[a] += 2;      // vertex planes a-3/2, a-1/2, a+1/2, a+3/2 around the centre
+                        const double m_m2 = face_mean(V, mv, a, lo2[0], lo2[1], lo2[2]);
+                        const double m_m1 = face_mean(V, mv, a, lo1[0], lo1[1], lo1[2]);
+                        const double m_p1 = face_mean(V, mv, a, hi1[0], hi1[1], hi1[2]);
+                        const double m_p2 = face_mean(V, mv, a, hi2[0], hi2[1], hi2[2]);
+                        dm[a][f] = (27.0 * (m_p1 - m_m1) - (m_p2 - m_m2)) / (24.0 * dx[a]);
+                    }
+                }
+                mc.alp = mcv[0];
+                for (int a = 0; a < 3; ++a) mc.beta[a] = mcv[1 + a];
+                for (int c = 0; c < 6; ++c) mc.g[c] = mcv[4 + c];
+                for (int c = 0; c < 6; ++c)
+                    K[c] = 0.5 * (face_mean(V, Kv + c * NV, 0, i, j, k) + face_mean(V, Kv + c * NV, 0, i + 1, j, k));
+                double P[8], S[8];
+                for (int q = 0; q < 8; ++q) P[q] = prim[q * NC + c0];
+                sources_point(P, mc, K, dm, gamma, S);
+                for (int c = 1; c <= 4; ++c) out[c * NC + c0] += S[c];
+            }
+    if (fallback_total) *fallback_total += nfb_all;
+    t_ops = {0, 0, 0, 0};
+}
+
+// R32: T^{mu nu} (Eq. 5, l.80-84) at the vertices of the interior cells.  The 8 primitives are interpolated from the cell
+// centres to the vertex with the tensor product of the symmetric 4-point midpoint rule (-1, 9, 9, -1)/16 (64 cells: "4th-
+// order symmetric 3D interpolation", l.84), then Eq. (5) is evaluated with the vertex's own metric sample:
+//   T^{mu nu} = rho h* u^mu u^nu + P* g^{mu nu} - b^mu b^nu,   u^0 = W/alpha, u^i = W (v^i - beta^i/alpha),
+//   b^0 = W B^k v_k / alpha, b^i = B^i / W + alpha b^0 (v^i - beta^i/alpha)... with b^i = (B^i + alpha b^0 u^i)/W,
+//   g^{00} = -1/alpha^2, g^{0i} = beta^i/alpha^2, g^{ij} = gamma^{ij} - beta^i beta^j/alpha^2.
+// T[10][vertex] = T^{00}, T^{0x}, T^{0y}, T^{0z}, T^{xx}, T^{xy}, T^{xz}, T^{yy}, T^{yz}, T^{zz}; vertices (0..n) per
+// direction (interior-cell corners); other entries untouched.  Needs 2 ghost cells.
+void tmunu_point(const double P[8], Metric<double>& m, double gamma, double T[10]) {
+    metric_complete(m);
+    const double rho = P[0], eps = P[4];
+    const double v[3] = {P[1], P[2], P[3]}, B[3] = {P[5], P[6], P[7]};
+    double vl[3], Bl[3];
+    for (int i = 0; i < 3; ++i) { vl[i] = lower(m, v, i); Bl[i] = lower(m, B, i); }
+    const double v2 = vl[0] * v[0] + vl[1] * v[1] + vl[2] * v[2];
+    const double W = 1.0 / std::sqrt(1.0 - v2);
+    const double Bv = Bl[0] * v[0] + Bl[1] * v[1] + Bl[2] * v[2];
+    const double B2 = Bl[0] * B[0] + Bl[1] * B[1] + Bl[2] * B[2];
+    const double a = m.alp;
+    double u[4], b[4];
+    u[0] = W / a;
+    for (int i = 0; i < 3; ++i) u[1 + i] = W * (v[i] - m.beta[i] / a);
+    b[0] = W * Bv / a;
+    for (int i = 0; i < 3; ++i) b[1 + i] = (B[i] + a * b[0] * u[1 + i]) / W;
+    const double b2 = (B2 + (a * b[0]) * (a * b[0])) / (W * W);
+    const double p = (gamma - 1.0) * rho * eps;
+    const double rhohs = rho * (1.0 + eps) + p + b2, Ps = p + 0.5 * b2;
+    double ginv[4][4];
+    ginv[0][0] = -1.0 / (a * a);
+    for (int i = 0; i < 3; ++i) ginv[0][1 + i] = ginv[1 + i][0] = m.beta[i] / (a * a);
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) ginv[1 + i][1 + j] = m.gu[SYM[i][j]] - m.beta[i] * m.beta[j] / (a * a);
+    int n = 0;
+    for (int mu = 0; mu < 4; ++mu)
+        for (int nu = mu; nu < 4; ++nu) T[n++] = rhohs * u[mu] * u[nu] + Ps * ginv[mu][nu] - b[mu] * b[nu];
+}
+
+void tmunu_vertex_box(const VGrid& V, const double* prim, const double* metv, double gamma, double* T) {
+    const Grid& G = V.G;
+    const size_t NC = G.ncell, NV = V.nv;
+    const double w[4] = {-1.0 / 16.0, 9.0 / 16.0, 9.0 / 16.0, -1.0 / 16.0};
+#pragma omp parallel for schedule(static) collapse(2)
+    for (int k = 0; k <= G.n[2]; ++k)
+        for (int j = 0; j <= G.n[1]; ++j)
+            for (int i = 0; i <= G.n[0]; ++i) {
+                double P[8];
+                for (int q = 0; q < 8; ++q) {
+                    double sum = 0.0;
+                    for (int c = 0; c < 4; ++c)
+                        for (int b = 0; b < 4; ++b)
+                            for (int a = 0; a < 4; ++a)
+                                sum += w[c] * w[b] * w[a] * prim[q * NC + G.idx(i - 2 + a, j - 2 + b, k - 2 + c)];
+                    P[q] = sum;
+                }
+                Metric<double> m;
+                const size_t v0 = V.vidx(i, j, k);
+                m.alp = metv[v0];
+                for (int a = 0; a < 3; ++a) m.beta[a] = metv[(1 + a) * NV + v0];
+                for (int c = 0; c < 6; ++c) m.g[c] = metv[(4 + c) * NV + v0];
+                double T10[10];
+                tmunu_point(P, m, gamma, T10);
+                for (int c = 0; c < 10; ++c) T[c * NV + v0] = T10[c];
+            }
+}
+
 }  // namespace
 
 // =================================================== C ABI ===================================================
@@ -962,6 +1153,42 @@ int oracle_flux_ct(const int n[3], int nbox, const double* FB, const double dx[3
     G.g = nghost;
     G.ncell = (size_t)G.N[0] * G.N[1] * G.N[2];
     for (int b = 0; b < nbox; ++b) flux_ct_box(G, FB + (size_t)b * 9 * G.ncell, dx, dB + (size_t)b * 3 * G.ncell);
+    return 0;
+}
+
+// NEXT-3: right-hand side with vertex-centred metric and K (metv [nbox][10][Nz+1][Ny+1][Nx+1], Kv [nbox][6][...]) and
+// T^{mu nu} at the vertices of the interior cells (T [nbox][10][Nz+1][Ny+1][Nx+1]).
+static bool make_vgrid(const int n[3], int nghost, VGrid& V) {
+    if (!n || n[0] < 1 || n[1] < 1 || n[2] < 1 || nghost < 0) return false;
+    for (int a = 0; a < 3; ++a) { V.G.n[a] = n[a]; V.G.N[a] = n[a] + 2 * nghost; }
+    V.G.g = nghost;
+    V.G.ncell = (size_t)V.G.N[0] * V.G.N[1] * V.G.N[2];
+    V.nv = (size_t)(V.G.N[0] + 1) * (V.G.N[1] + 1) * (V.G.N[2] + 1);
+    return true;
+}
+
+int oracle_valencia_rhs_vertex(const int n[3], int nbox, const double* prim, const double* metv, const double* Kv,
+                               const double dx[3], int nghost, int recon, double gamma, double* out,
+                               unsigned long long* nfallback) {
+    VGrid V;
+    if (!make_vgrid(n, nghost, V) || !prim || !metv || !Kv || !dx || !out || nbox < 1) return 1;
+    if (recon != RECON_MINMOD && recon != RECON_MC && recon != RECON_WENO5) return 1;
+    if (nghost < (recon == RECON_WENO5 ? 3 : 2)) return 1;
+    if (!(gamma > 1.0) || !(dx[0] > 0.0) || !(dx[1] > 0.0) || !(dx[2] > 0.0)) return 1;
+    unsigned long long nfb = 0;
+    for (int b = 0; b < nbox; ++b)
+        rhs_vertex_box(V, prim + (size_t)b * 8 * V.G.ncell, metv + (size_t)b * 10 * V.nv, Kv + (size_t)b * 6 * V.nv, dx, recon,
+                       gamma, out + (size_t)b * 8 * V.G.ncell, &nfb);
+    if (nfallback) *nfallback = nfb;
+    return 0;
+}
+
+int oracle_tmunu_vertices(const int n[3], int nbox, const double* prim, const double* metv, int nghost, double gamma,
+                          double* T) {
+    VGrid V;
+    if (!make_vgrid(n, nghost, V) || !prim || !metv || !T || nbox < 1 || nghost < 2 || !(gamma > 1.0)) return 1;
+    for (int b = 0; b < nbox; ++b)
+        tmunu_vertex_box(V, prim + (size_t)b * 8 * V.G.ncell, metv + (size_t)b * 10 * V.nv, gamma, T + (size_t)b * 10 * V.nv);
     return 0;
 }
 

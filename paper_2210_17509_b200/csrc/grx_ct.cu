@@ -55,9 +55,9 @@ __global__ void __launch_bounds__(128) face_bflux_kernel(const RhsParams p, cons
 
 // One thread per interior cell: twelve edge EMFs around the cell, replaced face fluxes, update of out[5..7].
 __global__ void __launch_bounds__(256) flux_ct_kernel(const RhsParams p) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = blockIdx.y * blockDim.x + threadIdx.x;
     if (i >= p.n[0]) return;
-    const int j = blockIdx.y % p.n[1], k = blockIdx.y / p.n[1];
+    const int j = blockIdx.x % p.n[1], k = blockIdx.x / p.n[1];     // rows in grid.x: up to 2^31 - 1 of them
     const int box = blockIdx.z;
     const long long nc = p.nc, sy = p.stride[1], sz = p.stride[2];
     const double* __restrict__ fb = p.fb + (long long)box * 6 * nc;
@@ -101,7 +101,7 @@ cudaError_t launch_flux_ct(const RhsParams& p, cudaStream_t st) {
     const long long rows = (long long)p.n[1] * p.n[2];
     if (rows > 2147483647LL) return cudaErrorInvalidConfiguration;
     const int bx = p.n[0] >= 256 ? 256 : (p.n[0] >= 128 ? 128 : (p.n[0] >= 64 ? 64 : 32));
-    const dim3 grid((unsigned)((p.n[0] + bx - 1) / bx), (unsigned)rows, p.nbox);
+    const dim3 grid((unsigned)rows, (unsigned)((p.n[0] + bx - 1) / bx), p.nbox);
     flux_ct_kernel<<<grid, bx, 0, st>>>(p);
     return cudaGetLastError();
 }
