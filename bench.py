@@ -361,6 +361,46 @@ def time_halo_overlap(grx, torch, prob, dev, recon, stream, world, nsteps=3):
     return res
 
 
+def time_vertex(grx, torch, prob, dev, recon, stream, steps=5):
+    """NEXT-3: grx_valencia_rhs_vertex (metric / K_ij at the cell vertices; here: the block's cell-centred fields sampled
+    onto the (N+1)^3 vertex grid by edge replication -- the timing does not depend on the values) and grx_tmunu_vertices."""
+    prim, met, K = dev
+
+    def to_vertices(a):
+        v = torch.empty((a.shape[0], a.shape[1]) + tuple(s + 1 for s in a.shape[2:]), dtype=a.dtype, device=a.device)
+        v[:, :, :-1, :-1, :-1] = a
+        v[:, :, -1, :-1, :-1] = a[:, :, -1]
+        v[:, :, :, -1, :-1] = v[:, :, :, -2, :-1]
+        v[:, :, :, :, -1] = v[:, :, :, :, -2]
+        return v
+
+    met_v, K_v = to_vertices(met), to_vertices(K)
+    out = torch.empty_like(prim)
+    T = torch.empty((prim.shape[0], 10) + tuple(met_v.shape[2:]), dtype=torch.float64, device="cuda")
+    res = {}
+    for name, call in (("rhs_vertex", lambda: grx.valencia_rhs_vertex(prim, met_v, K_v, prob.dx, prob.nghost, recon, prob.gamma,
+                                                                      out=out, stream=stream)),
+                       ("tmunu_vertices", lambda: grx.tmunu_vertices(prim, met_v, prob.nghost, prob.gamma, out=T, stream=stream))):
+        for _ in range(2):
+            call()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        stream.synchronize()
+        e0.record(stream)
+        for _ in range(steps):
+            call()
+        e1.record(stream)
+        stream.synchronize()
+        t = e0.elapsed_time(e1) * 1e-3 / steps
+        res[name] = {"ms_per_call": 1e3 * t, "cell_updates_per_s": prob.cells / t}
+    fl = algorithmic_flops_per_cell(prob.n, recon) * prob.cells / (res["rhs_vertex"]["ms_per_call"] * 1e-3) / 1e12
+    res["rhs_vertex"]["frac_of_cell_centred_count"] = fl / FP64_PEAK_NOMINAL_TFLOPS
+    # T^{mu nu}: 8 prims read (cached 64-point stencils), 10 metric fields read, 10 components written per vertex
+    res["tmunu_vertices"]["hbm_frac"] = 28 * 8 * prob.cells / (res["tmunu_vertices"]["ms_per_call"] * 1e-3) / 1e9 / \
+        measured_peaks()[0].get("hbm_gbs", 6650.0)
+    res["scheme"] = f"metric and K_ij at the cell vertices (R31), T^mu nu from 4th-order interpolated primitives (R32); {prob.name}"
+    return res
+
+
 def measure_dfma_peak(grx, torch, stream):
     sink = torch.zeros(1, dtype=torch.float64, device="cuda")
     grx.dfma_peak_launch(2000, sink, stream)
@@ -530,10 +570,11 @@ def run_ours(args):
 
     # ---- NEXT-1: device-resident time steps on the same block (context: the paper's setupA, l.329-341: static spacetime,
     # ideal gas, RK2, WENO5, periodic boundaries, 3 ghosts -> 0.47e8 zone-cycles/s at 240^3 on one V100)
-    zone_cycles = ct = None
+    zone_cycles = ct = vertex = None
     if not args.no_sweep:
         zone_cycles = time_zone_cycles(grx, torch, prob, dev, recon, stream)
         ct = time_ct(grx, torch, prob, dev, recon, stream)
+        vertex = time_vertex(grx, torch, prob, dev, recon, stream)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -556,6 +597,8 @@ def run_ours(args):
         line["zone_cycles"] = zone_cycles
     if ct is not None:
         line["constrained_transport"] = ct
+    if vertex is not None:
+        line["vertex_centred"] = vertex
     if halo_res is not None:
         line["halo_overlap"] = halo_res
     print(json.dumps(line), flush=True)

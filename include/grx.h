@@ -184,6 +184,24 @@ int grx_rk_stage(const grx_grid* grid, int nghost, double a, const double* Ua, d
                  const double* L, double* Uout, double* acc, double wdt, const double* metric, double gamma, double* prim,
                  unsigned long long* nfail, void* cuda_stream);
 
+/* NEXT-3: the paper's own centring of the spacetime fields -- "stored on vertices",
+ * "known at the cell vertices and ... interpolated linearly to the face centers" (l.130); T^{mu nu} "stored as samples at the
+ * cell vertices" from fluid variables brought there by "a 4th-order symmetric 3D interpolation" (l.84, l.323).  Readings R31 /
+ * R32.  Vertex arrays: metric_v[nbox][10][Nz+1][Ny+1][Nx+1], K_v[nbox][6][Nz+1][Ny+1][Nx+1], vertex (I, J, K) = the
+ * low corner of cell (I, J, K) (indices with ghosts).
+ *
+ * grx_valencia_rhs_vertex: grx_valencia_rhs with face metric = mean of the 4 vertices of the face, cell-centre metric and K_ij
+ *   = mean of the 8 vertices of the cell, metric derivatives = [27 (m(+1/2) - m(-1/2)) - (m(+3/2) - m(-3/2))] / (24 dx) of the
+ *   transverse 4-vertex means.  prim, dx, nghost, recon, gamma, out, errors: as for grx_valencia_rhs.
+ * grx_tmunu_vertices: T[nbox][10][Nz+1][Ny+1][Nx+1] = T^{00}, T^{0x}, T^{0y}, T^{0z}, T^{xx}, T^{xy}, T^{xz}, T^{yy}, T^{yz}, T^{zz}
+ *   (Eq. 5, l.80) at the (n+1)^3 vertices of the interior cells of every box; other entries are not written.  The 8
+ *   primitives are interpolated to the vertex with the tensor product of (-1, 9, 9, -1)/16 over the 4 x 4 x 4 cells around it
+ *   (nghost >= 2), the metric is the vertex's own sample. */
+int grx_valencia_rhs_vertex(const grx_grid* grid, const double* prim, const double* metric_v, const double* K_v,
+                            const double dx[3], int nghost, int recon, double gamma, double* out, void* cuda_stream);
+int grx_tmunu_vertices(const grx_grid* grid, const double* prim, const double* metric_v, int nghost, double gamma, double* T,
+                       void* cuda_stream);
+
 /* Debug: if `counter` (DEVICE pointer to one unsigned long long, caller-zeroed) is non-NULL, later
  * grx_valencia_rhs calls of this host thread add to it the number of face sides that took the R5
  * first-order fallback.  NULL switches counting off (the default; counting costs a few atomics). */

@@ -15,7 +15,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgrx.so")
 OBJDIR = os.path.join(ROOT, "build", "grx")
-SOURCES = ["grx_api.cu", "grx_simple.cu", "grx_fused.cu", "grx_tma.cu", "grx_ct.cu", "grx_support.cu"]
+SOURCES = ["grx_api.cu", "grx_simple.cu", "grx_fused.cu", "grx_tma.cu", "grx_ct.cu", "grx_vertex.cu", "grx_support.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--fmad=true",

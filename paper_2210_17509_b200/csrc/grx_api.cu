@@ -379,6 +379,45 @@ int grx_halo_z(const grx_grid* grid, double* prim, int nghost, int side, int unp
     return GRX_OK;
 }
 
+int grx_valencia_rhs_vertex(const grx_grid* grid, const double* prim, const double* metric_v, const double* K_v,
+                            const double dx[3], int nghost, int recon, double gamma, double* out, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim || !metric_v || !K_v || !dx || !out) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (recon != GRX_RECON_MINMOD && recon != GRX_RECON_MC && recon != GRX_RECON_WENO5)
+        return fail(GRX_ERR_INVALID_ARG, "unknown recon");
+    if (nghost < (recon == GRX_RECON_WENO5 ? 3 : 2))
+        return fail(GRX_ERR_INVALID_ARG, "nghost too small: WENO5 needs 3, minmod/MC need 2 (R29)");
+    if (!(gamma > 1.0)) return fail(GRX_ERR_INVALID_ARG, "gamma must be > 1");
+    for (int a = 0; a < 3; ++a) {
+        if (!(dx[a] > 0.0) || !(1.0 / dx[a] > 0.0)) return fail(GRX_ERR_INVALID_ARG, "dx must be > 0 and finite");
+        p.idx[a] = 1.0 / dx[a];
+    }
+    if (out == prim) return fail(GRX_ERR_INVALID_ARG, "out must not alias an input");
+    p.prim = prim; p.met = metric_v; p.K = K_v; p.out = out;
+    p.gamma = gamma;
+    p.nfallback = t_fallback_counter;
+    const cudaError_t e = grx::launch_rhs_vertex(p, recon, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_vertex launch");
+    return GRX_OK;
+}
+
+int grx_tmunu_vertices(const grx_grid* grid, const double* prim, const double* metric_v, int nghost, double gamma, double* T,
+                       void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim || !metric_v || !T) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (nghost < 2) return fail(GRX_ERR_INVALID_ARG, "the 4-point interpolation needs 2 ghost cells");
+    if (!(gamma > 1.0)) return fail(GRX_ERR_INVALID_ARG, "gamma must be > 1");
+    p.prim = prim; p.met = metric_v;
+    p.gamma = gamma;
+    const cudaError_t e = grx::launch_tmunu_vertex(p, T, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_tmunu_vertices launch");
+    return GRX_OK;
+}
+
 size_t grx_ct_workspace_bytes(const grx_grid* grid, int nghost) {
     grx::RhsParams p;
     std::memset(&p, 0, sizeof(p));

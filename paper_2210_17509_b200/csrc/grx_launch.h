@@ -23,6 +23,10 @@ double tma_tile_efficiency(const RhsParams& p, int sms);
 cudaError_t launch_face_bflux(const RhsParams& p, int recon, bool all, cudaStream_t st);
 cudaError_t launch_flux_ct(const RhsParams& p, cudaStream_t st);
 
+// grx_vertex.cu: NEXT-3, metric and K_ij sampled at the cell vertices (p.met / p.K point at vertex arrays)
+cudaError_t launch_rhs_vertex(const RhsParams& p, int recon, cudaStream_t st);
+cudaError_t launch_tmunu_vertex(const RhsParams& p, double* T, cudaStream_t st);
+
 // grx_support.cu
 cudaError_t launch_prim2con(const double* prim, const double* met, long long nc, int nbox, double gamma, double* cons,
                             cudaStream_t st);

@@ -19,7 +19,7 @@ VARIANT = {"auto": 0, "simple": 1, "ldg": 2, "tma": 3}
 EXPORTS = (
     "grx_valencia_rhs", "grx_valencia_rhs_host", "grx_host_workspace_bytes", "grx_prim2con", "grx_con2prim", "grx_rk_axpy",
     "grx_step_rk", "grx_step_workspace_bytes", "grx_valencia_rhs_ct", "grx_ct_workspace_bytes",
-    "grx_valencia_rhs_zrange", "grx_halo_z", "grx_halo_z_bytes", "grx_fill_ghosts", "grx_rk_stage", "grx_debug_set_fallback_counter",
+    "grx_valencia_rhs_vertex", "grx_tmunu_vertices", "grx_valencia_rhs_zrange", "grx_halo_z", "grx_halo_z_bytes", "grx_fill_ghosts", "grx_rk_stage", "grx_debug_set_fallback_counter",
     "grx_set_variant", "grx_selftest_math", "grx_dfma_peak_launch", "grx_fp64_issue_probe", "grx_last_error", "grx_version",
     "grx_weno_eps", "grx_v2max",
 )
@@ -62,6 +62,8 @@ def lib():
         L.grx_halo_z.argtypes = [gp, vp, i, i, i, vp, vp]
         L.grx_fill_ghosts.argtypes = [gp, vp, i, i, i, vp]
         L.grx_rk_stage.argtypes = [gp, i, dbl, vp, dbl, vp, dbl, vp, vp, vp, dbl, vp, dbl, vp, vp, vp]
+        L.grx_valencia_rhs_vertex.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, vp]
+        L.grx_tmunu_vertices.argtypes = [gp, vp, vp, i, dbl, vp, vp]
         L.grx_debug_set_fallback_counter.argtypes = [vp]
         L.grx_set_variant.argtypes = [i]
         L.grx_selftest_math.argtypes = [vp, vp, sz, vp]
@@ -271,6 +273,41 @@ def rk_stage(nghost, a, Ua, b, Ub, h, L, Uout, metric, gamma, prim, acc=None, wd
                               _dev(Uout, 8), _dev(acc, 8) if acc is not None else nul, float(wdt), _dev(metric, 10),
                               float(gamma), _dev(prim, 8), C.c_void_p(nfail.data_ptr()) if nfail is not None else nul,
                               _stream(stream)))
+
+
+def _devv(t, nfield, prim):
+    """A vertex array [nbox, nfield, Nz+1, Ny+1, Nx+1] that belongs to `prim`."""
+    import torch
+    want = (prim.shape[0], nfield) + tuple(s + 1 for s in prim.shape[2:])
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()) \
+            or tuple(t.shape) != want:
+        raise GrxError(f"expected a contiguous CUDA float64 vertex array of shape {want}")
+    return C.c_void_p(t.data_ptr())
+
+
+def valencia_rhs_vertex(prim, metric_v, K_v, dx, nghost, recon, gamma, out=None, stream=None):
+    """grx_valencia_rhs_vertex (NEXT-3): the right-hand side with metric and K_ij sampled at the cell vertices."""
+    import torch
+    if out is None:
+        out = torch.empty_like(prim)
+    g = _grid(prim, nghost)
+    r = RECON[recon] if isinstance(recon, str) else int(recon)
+    dxa = (C.c_double * 3)(*[float(v) for v in dx])
+    _check(lib().grx_valencia_rhs_vertex(C.byref(g), _dev(prim, 8), _devv(metric_v, 10, prim), _devv(K_v, 6, prim), dxa,
+                                         int(nghost), r, float(gamma), _dev(out, 8), _stream(stream)))
+    return out
+
+
+def tmunu_vertices(prim, metric_v, nghost, gamma, out=None, stream=None):
+    """grx_tmunu_vertices (NEXT-3): T^{mu nu} [nbox, 10, Nz+1, Ny+1, Nx+1] at the vertices of the interior cells."""
+    import torch
+    if out is None:
+        out = torch.full((prim.shape[0], 10) + tuple(s + 1 for s in prim.shape[2:]), float("nan"), dtype=torch.float64,
+                         device=prim.device)
+    g = _grid(prim, nghost)
+    _check(lib().grx_tmunu_vertices(C.byref(g), _dev(prim, 8), _devv(metric_v, 10, prim), int(nghost), float(gamma),
+                                    _devv(out, 10, prim), _stream(stream)))
+    return out
 
 
 def set_fallback_counter(counter):
