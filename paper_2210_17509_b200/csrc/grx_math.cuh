@@ -442,9 +442,23 @@ GRX_HD void prim2con_point(const double P[8], const double met[10], double gamma
     U[5] = sg * Bx; U[6] = sg * By; U[7] = sg * Bz;
 }
 
-// ---- support (R22): Gamma-law con2prim at one point, Newton on z = rho h W^2 with a bracket -----------------
-// Returns 0 on convergence, 1 otherwise.
-GRX_HD int con2prim_point(const double U[8], const double met[10], double gamma, double P[8]) {
+// ---- support (R22): Gamma-law con2prim at one point, Newton on z = rho h W^2 ----------------------------------
+// f(z) = z + B^2 - p(z) - B^2/(2 W^2) - (S.B)^2/(2 z^2) - (tau + D) on the undensitised conserved variables, with
+// v^2(z) = [S^2 z^2 + (S.B)^2 (B^2 + 2z)] / [(z + B^2)^2 z^2].
+struct C2P {
+    double Dd, E, S2, B2, SB, SB2, gamma;
+    double Su[3], B[3];
+    double W, rho, p;    // of the last eval
+    GRX_HD double eval(double z) {
+        double v2 = (S2 * z * z + SB2 * (B2 + 2.0 * z)) / ((z + B2) * (z + B2) * z * z);
+        if (v2 > 1.0 - 1e-15) v2 = 1.0 - 1e-15;
+        W = 1.0 / sqrt(1.0 - v2);
+        rho = Dd / W;
+        p = (gamma - 1.0) / gamma * (z / (W * W) - rho);
+        return z + B2 - p - B2 / (2.0 * W * W) - SB2 / (2.0 * z * z) - E;
+    }
+};
+GRX_HD void con2prim_setup(const double U[8], const double met[10], double gamma, C2P& s) {
     const double gxx = met[4], gxy = met[5], gxz = met[6], gyy = met[7], gyz = met[8], gzz = met[9];
     const double cxx = fma(gyy, gzz, -gyz * gyz);
     const double cxy = fma(gxz, gyz, -gxy * gzz);
@@ -454,54 +468,102 @@ GRX_HD int con2prim_point(const double U[8], const double met[10], double gamma,
     const double czz = fma(gxx, gyy, -gxy * gxy);
     const double det = fma(gxx, cxx, fma(gxy, cxy, gxz * cxz));
     const double isg = 1.0 / sqrt(det), idet = 1.0 / det;
-    const double Dd = U[0] * isg, tau = U[4] * isg;
+    s.Dd = U[0] * isg;
+    const double tau = U[4] * isg;
     const double Slx = U[1] * isg, Sly = U[2] * isg, Slz = U[3] * isg;
-    const double Bx = U[5] * isg, By = U[6] * isg, Bz = U[7] * isg;
-    const double Sux = (cxx * Slx + cxy * Sly + cxz * Slz) * idet;
-    const double Suy = (cxy * Slx + cyy * Sly + cyz * Slz) * idet;
-    const double Suz = (cxz * Slx + cyz * Sly + czz * Slz) * idet;
-    const double Blx = gxx * Bx + gxy * By + gxz * Bz;
-    const double Bly = gxy * Bx + gyy * By + gyz * Bz;
-    const double Blz = gxz * Bx + gyz * By + gzz * Bz;
-    const double S2 = Slx * Sux + Sly * Suy + Slz * Suz;
-    const double B2 = Blx * Bx + Bly * By + Blz * Bz;
-    const double SB = Slx * Bx + Sly * By + Slz * Bz;
-    const double E = tau + Dd;
-    const double SB2 = SB * SB;
-    double W = 1.0, rho = Dd, p = 0.0;
-    auto eval = [&](double z) {
-        double v2 = (S2 * z * z + SB2 * (B2 + 2.0 * z)) / ((z + B2) * (z + B2) * z * z);
-        if (v2 > 1.0 - 1e-15) v2 = 1.0 - 1e-15;
-        W = 1.0 / sqrt(1.0 - v2);
-        rho = Dd / W;
-        p = (gamma - 1.0) / gamma * (z / (W * W) - rho);
-        return z + B2 - p - B2 / (2.0 * W * W) - SB2 / (2.0 * z * z) - E;
-    };
-    double zhi = fmax(2.0 * (E + 1.0), 1.0);
-    for (int it = 0; it < 200 && eval(zhi) < 0.0; ++it) zhi *= 2.0;
+    s.B[0] = U[5] * isg; s.B[1] = U[6] * isg; s.B[2] = U[7] * isg;
+    s.Su[0] = (cxx * Slx + cxy * Sly + cxz * Slz) * idet;
+    s.Su[1] = (cxy * Slx + cyy * Sly + cyz * Slz) * idet;
+    s.Su[2] = (cxz * Slx + cyz * Sly + czz * Slz) * idet;
+    const double Blx = gxx * s.B[0] + gxy * s.B[1] + gxz * s.B[2];
+    const double Bly = gxy * s.B[0] + gyy * s.B[1] + gyz * s.B[2];
+    const double Blz = gxz * s.B[0] + gyz * s.B[1] + gzz * s.B[2];
+    s.S2 = Slx * s.Su[0] + Sly * s.Su[1] + Slz * s.Su[2];
+    s.B2 = Blx * s.B[0] + Bly * s.B[1] + Blz * s.B[2];
+    s.SB = Slx * s.B[0] + Sly * s.B[1] + Slz * s.B[2];
+    s.SB2 = s.SB * s.SB;
+    s.E = tau + s.Dd;
+    s.gamma = gamma;
+    s.W = 1.0; s.rho = s.Dd; s.p = 0.0;
+}
+GRX_HD void con2prim_finish(C2P& s, double z, double P[8]) {
+    s.eval(z);
+    P[0] = s.rho;
+    const double iz = 1.0 / z, izb = 1.0 / (z + s.B2);
+    P[1] = (s.Su[0] + s.SB * s.B[0] * iz) * izb;
+    P[2] = (s.Su[1] + s.SB * s.B[1] * iz) * izb;
+    P[3] = (s.Su[2] + s.SB * s.B[2] * iz) * izb;
+    P[4] = s.p / ((s.gamma - 1.0) * s.rho);
+    P[5] = s.B[0]; P[6] = s.B[1]; P[7] = s.B[2];
+}
+// Bracketed solve: grow / shrink a bracket from 2 (E + 1), then Newton with a central-difference slope, bisecting whenever
+// a step leaves the bracket.  Returns 0 on convergence (|dz| < 1e-14 z), 1 otherwise.
+GRX_HD int con2prim_solve_bracket(C2P& s, double& zout) {
+    double zhi = fmax(2.0 * (s.E + 1.0), 1.0);
+    for (int it = 0; it < 200 && s.eval(zhi) < 0.0; ++it) zhi *= 2.0;
     double zlo = zhi;
-    for (int it = 0; it < 400 && eval(zlo) > 0.0; ++it) zlo *= 0.5;
+    for (int it = 0; it < 400 && s.eval(zlo) > 0.0; ++it) zlo *= 0.5;
     double z = 0.5 * (zlo + zhi);
     int status = 1;
     for (int it = 0; it < 200; ++it) {
-        const double f = eval(z);
+        const double f = s.eval(z);
         if (f > 0.0) zhi = z; else zlo = z;
         const double h = 1e-6 * z;
-        const double fp = (eval(z + h) - eval(z - h)) / (2.0 * h);
+        const double fp = (s.eval(z + h) - s.eval(z - h)) / (2.0 * h);
         double zn = z - f / fp;
         if (!(zn > zlo && zn < zhi)) zn = 0.5 * (zlo + zhi);
         const double dz = fabs(zn - z);
         z = zn;
         if (dz < 1e-14 * z) { status = 0; break; }
     }
-    eval(z);
-    P[0] = rho;
-    const double iz = 1.0 / z, izb = 1.0 / (z + B2);
-    P[1] = (Sux + SB * Bx * iz) * izb;
-    P[2] = (Suy + SB * By * iz) * izb;
-    P[3] = (Suz + SB * Bz * iz) * izb;
-    P[4] = p / ((gamma - 1.0) * rho);
-    P[5] = Bx; P[6] = By; P[7] = Bz;
+    zout = z;
+    return status;
+}
+// Warm-started solve for time stepping: the old state's z = rho h W^2 is within a time step of the root, so one Newton
+// step with a central-difference slope followed by secant steps (one evaluation each) reaches |dz| < 1e-14 z in a handful of
+// evaluations.  Returns 0 on convergence; anything else (no convergence in 12 steps, a step to z <= 0 or NaN) makes the
+// caller take the bracketed solve.
+GRX_HD int con2prim_solve_warm(C2P& s, double z0, double& zout) {
+    if (!(z0 > 0.0)) return 1;
+    double z = z0, f0 = s.eval(z);
+    const double h = 1e-6 * z;
+    double slope = (s.eval(z + h) - s.eval(z - h)) / (2.0 * h);
+    for (int it = 0; it < 12; ++it) {
+        const double zn = z - f0 / slope;
+        if (!(zn > 0.0)) return 1;
+        const double dz = fabs(zn - z);
+        if (dz < 1e-14 * zn) { zout = zn; return 0; }
+        const double f1 = s.eval(zn);
+        const double sl = (f1 - f0) / (zn - z);
+        if (sl > 0.0) slope = sl;      // f is increasing at the root: a secant slope of the wrong sign is rounding noise
+        z = zn;
+        f0 = f1;
+    }
+    return 1;
+}
+// Returns 0 on convergence, 1 otherwise.
+GRX_HD int con2prim_point(const double U[8], const double met[10], double gamma, double P[8]) {
+    C2P s;
+    con2prim_setup(U, met, gamma, s);
+    double z;
+    const int status = con2prim_solve_bracket(s, z);
+    con2prim_finish(s, z, P);
+    return status;
+}
+// Pold: the primitives of the same cell at the previous stage (the warm start); falls back to the bracketed solve.
+GRX_HD int con2prim_point_warm(const double U[8], const double met[10], double gamma, const double Pold[8], double P[8]) {
+    C2P s;
+    con2prim_setup(U, met, gamma, s);
+    // z of the old state: rho h W^2 with v^2 = gamma_ij v^i v^j
+    const double gxx = met[4], gxy = met[5], gxz = met[6], gyy = met[7], gyz = met[8], gzz = met[9];
+    const double vx = Pold[1], vy = Pold[2], vz = Pold[3];
+    const double v2 = vx * (gxx * vx + gxy * vy + gxz * vz) + vy * (gxy * vx + gyy * vy + gyz * vz) +
+                      vz * (gxz * vx + gyz * vy + gzz * vz);
+    const double z0 = Pold[0] * (1.0 + gamma * Pold[4]) / (1.0 - v2);
+    double z;
+    int status = con2prim_solve_warm(s, z0, z);
+    if (status) status = con2prim_solve_bracket(s, z);
+    con2prim_finish(s, z, P);
     return status;
 }
 

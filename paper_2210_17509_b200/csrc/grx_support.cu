@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(128) rk_stage_kernel(const __grid_constant__ R
     const long long c0 = (i + p.g) + p.stride[1] * (j + p.g) + p.stride[2] * (k + p.g);
     const long long ub = (long long)blockIdx.y * 8 * p.nc + c0;
     const double* mb = p.met + (long long)blockIdx.y * 10 * p.nc + c0;
-    double U[8], P[8], m[10];
+    double U[8], P[8], Pold[8], m[10];
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
         const long long o = ub + c * p.nc;
@@ -80,10 +80,11 @@ __global__ void __launch_bounds__(128) rk_stage_kernel(const __grid_constant__ R
         U[c] = a * Ua[o] + b * (Ub[o] + h * l);
         Uout[o] = U[c];
         if (acc) acc[o] += wdt * l;
+        Pold[c] = prim[o];      // the state the stage started from: warm start of the solve
     }
 #pragma unroll
     for (int f = 0; f < 10; ++f) m[f] = mb[f * p.nc];
-    const int bad = con2prim_point(U, m, p.gamma, P);
+    const int bad = con2prim_point_warm(U, m, p.gamma, Pold, P);
 #pragma unroll
     for (int c = 0; c < 8; ++c) prim[ub + c * p.nc] = P[c];
     if (bad && nfail) atomicAdd(nfail, 1ULL);

@@ -121,5 +121,15 @@ void hm_recon_cell(int recon, const double q[5], double* qm, double* qp) {
 
 void hm_prim2con(const double P[8], const double met[10], double gamma, double U[8]) { prim2con_point(P, met, gamma, U); }
 int hm_con2prim(const double U[8], const double met[10], double gamma, double P[8]) { return con2prim_point(U, met, gamma, P); }
+int hm_con2prim_warm(const double U[8], const double met[10], double gamma, const double Pold[8], double P[8]) {
+    return con2prim_point_warm(U, met, gamma, Pold, P);
+}
+// evaluations the warm solve needs from the old state Pold (-1: it gave up and the caller falls back to the bracket)
+int hm_con2prim_warm_steps(const double U[8], const double met[10], double gamma, double z0) {
+    C2P s;
+    con2prim_setup(U, met, gamma, s);
+    double z;
+    return con2prim_solve_warm(s, z0, z) == 0 ? 0 : -1;
+}
 
 }  // extern "C"

@@ -88,3 +88,28 @@ def test_prim2con_con2prim_pointwise(hm, oracle):
         back = np.empty(8)
         assert hm.hm_con2prim(_p(U), _p(met), C.c_double(1.6), _p(back)) == 0
         assert np.abs(back - P).max() < 1e-11
+
+
+def test_con2prim_warm_start_agrees_with_the_bracketed_solve(hm):
+    """The RK stage kernel starts the solve from the previous stage's primitives (con2prim_point_warm): from a state a few
+    per cent away it converges to the bracketed solve's answer; a useless guess (negative, NaN, far off) falls back to it."""
+    rng = np.random.default_rng(8)
+    hm.hm_con2prim.restype = C.c_int
+    hm.hm_con2prim_warm.restype = C.c_int
+    hm.hm_con2prim_warm_steps.restype = C.c_int
+    met = np.array([0.9, 0.01, -0.02, 0.03, 1.3, 0.1, -0.05, 1.1, 0.02, 0.9])
+    ok_warm = 0
+    for _ in range(200):
+        P = np.array([rng.uniform(0.1, 2), *rng.uniform(-0.4, 0.4, 3), rng.uniform(0.1, 3), *rng.uniform(-1, 1, 3)])
+        U, a, b = np.empty(8), np.empty(8), np.empty(8)
+        hm.hm_prim2con(_p(P), _p(met), C.c_double(1.6), _p(U))
+        assert hm.hm_con2prim(_p(U), _p(met), C.c_double(1.6), _p(a)) == 0
+        Pold = P * (1 + 0.05 * rng.uniform(-1, 1, 8))
+        assert hm.hm_con2prim_warm(_p(U), _p(met), C.c_double(1.6), _p(Pold), _p(b)) == 0
+        assert np.abs(a - b).max() < 1e-12
+        rhoh = Pold[0] * (1 + 1.6 * Pold[4])
+        ok_warm += hm.hm_con2prim_warm_steps(_p(U), _p(met), C.c_double(1.6), C.c_double(rhoh)) == 0
+        for bad in (np.full(8, np.nan), -P, P * 1e6):
+            assert hm.hm_con2prim_warm(_p(U), _p(met), C.c_double(1.6), _p(bad), _p(b)) == 0
+            assert np.abs(a - b).max() < 1e-12
+    assert ok_warm >= 195          # the warm path itself converges (it is not the fallback doing the work)
