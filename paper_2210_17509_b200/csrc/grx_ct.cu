@@ -22,12 +22,40 @@ template <int RECON>
 __global__ void __launch_bounds__(128) face_bflux_kernel(const RhsParams p, const int all) {
     const int ex = p.n[0] + 2, ey = p.n[1] + 2;
     long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long per_box = (long long)ex * ey * (p.n[2] + 2);
-    if (t >= per_box) return;
     const int box = blockIdx.y;
-    const int i = (int)(t % ex) - 1;
-    t /= ex;
-    const int j = (int)(t % ey) - 1, k = (int)(t / ey) - 1;
+    int i, j, k;
+    if (all) {
+        const long long per_box = (long long)ex * ey * (p.n[2] + 2);
+        if (t >= per_box) return;
+        i = (int)(t % ex) - 1;
+        t /= ex;
+        j = (int)(t % ey) - 1;
+        k = (int)(t / ey) - 1;
+    } else {
+        // the cells with an index outside [0, n) only, enumerated region by region so that warps are full:
+        // A: the two planes k = -1, n;  B: the rows j = -1, n of the planes between;  C: the columns i = -1, n of the rest
+        const long long nA = 2LL * ex * ey, nB = 2LL * ex * p.n[2], nC = 2LL * p.n[1] * p.n[2];
+        if (t < nA) {
+            i = (int)(t % ex) - 1;
+            t /= ex;
+            j = (int)(t % ey) - 1;
+            k = (t / ey) ? p.n[2] : -1;
+        } else if (t < nA + nB) {
+            t -= nA;
+            i = (int)(t % ex) - 1;
+            t /= ex;
+            k = (int)(t % p.n[2]);
+            j = (t / p.n[2]) ? p.n[1] : -1;
+        } else if (t < nA + nB + nC) {
+            t -= nA + nB;
+            j = (int)(t % p.n[1]);
+            t /= p.n[1];
+            k = (int)(t % p.n[2]);
+            i = (t / p.n[2]) ? p.n[0] : -1;
+        } else {
+            return;
+        }
+    }
     const bool ix = (i >= 0 && i < p.n[0]), iy = (j >= 0 && j < p.n[1]), iz = (k >= 0 && k < p.n[2]);   // interior index
     const double* __restrict__ prim = p.prim + (long long)box * 8 * p.nc;
     const double* __restrict__ met = p.met + (long long)box * 10 * p.nc;
@@ -89,8 +117,9 @@ __global__ void __launch_bounds__(256) flux_ct_kernel(const RhsParams p) {
 }  // namespace
 
 cudaError_t launch_face_bflux(const RhsParams& p, int recon, bool all, cudaStream_t st) {
-    const long long per_box = (long long)(p.n[0] + 2) * (p.n[1] + 2) * (p.n[2] + 2);
-    const dim3 grid((unsigned)((per_box + 127) / 128), p.nbox);
+    const long long ex = p.n[0] + 2, ey = p.n[1] + 2;
+    const long long threads = all ? ex * ey * (p.n[2] + 2) : 2 * ex * ey + 2 * ex * p.n[2] + 2LL * p.n[1] * p.n[2];
+    const dim3 grid((unsigned)((threads + 127) / 128), p.nbox);
     if (recon == RECON_WENO5) face_bflux_kernel<RECON_WENO5><<<grid, 128, 0, st>>>(p, all ? 1 : 0);
     else if (recon == RECON_MC) face_bflux_kernel<RECON_MC><<<grid, 128, 0, st>>>(p, all ? 1 : 0);
     else face_bflux_kernel<RECON_MINMOD><<<grid, 128, 0, st>>>(p, all ? 1 : 0);
