@@ -9,8 +9,9 @@
 //
 // Parity pins: every exported function below is pinned by tests/test_oracle_pins*.py against
 // closed forms, invariants and the paper's printed Balsara-1 values (tests/golden/).  Conventions
-// that no external value can pin -- WENO_EPS, V2MAX, the fast-speed approximation a^2 (R8) and
-// the MC limiter -- are listed as "parity unpinned (convention)" in DESIGN.md.
+// that no external value can pin -- WENO_EPS, V2MAX, the fast-speed approximation a^2 (R8), the MC
+// limiter and the choice of flux-CT among the constrained-transport schemes (R30; its defining
+// properties are pinned) -- are listed as "parity unpinned (convention)" in DESIGN.md.
 //
 // No blocking, fusion or re-ordering beyond what the algorithm states: per direction, per grid
 // line: reconstruct (O2) -> face metric (O1) -> admissibility (O3) -> state (O4) -> flux (O5)
