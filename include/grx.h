@@ -192,7 +192,8 @@ int grx_rk_stage(const grx_grid* grid, int nghost, double a, const double* Ua, d
  *
  * grx_valencia_rhs_vertex: grx_valencia_rhs with face metric = mean of the 4 vertices of the face, cell-centre metric and K_ij
  *   = mean of the 8 vertices of the cell, metric derivatives = [27 (m(+1/2) - m(-1/2)) - (m(+3/2) - m(-3/2))] / (24 dx) of the
- *   transverse 4-vertex means.  prim, dx, nghost, recon, gamma, out, errors: as for grx_valencia_rhs.
+ *   transverse 4-vertex means.  prim, dx, nghost, recon, gamma, out, errors: as for grx_valencia_rhs.  Runs on the tile
+ *   traversal of the LDG kernel with vertex loads (GRX_VARIANT_SIMPLE: one thread per cell, the cross-check).
  * grx_tmunu_vertices: T[nbox][10][Nz+1][Ny+1][Nx+1] = T^{00}, T^{0x}, T^{0y}, T^{0z}, T^{xx}, T^{xy}, T^{xz}, T^{yy}, T^{yz}, T^{zz}
  *   (Eq. 5, l.80) at the (n+1)^3 vertices of the interior cells of every box; other entries are not written.  The 8
  *   primitives are interpolated to the vertex with the tensor product of (-1, 9, 9, -1)/16 over the 4 x 4 x 4 cells around it

@@ -398,7 +398,11 @@ int grx_valencia_rhs_vertex(const grx_grid* grid, const double* prim, const doub
     p.prim = prim; p.met = metric_v; p.K = K_v; p.out = out;
     p.gamma = gamma;
     p.nfallback = t_fallback_counter;
-    const cudaError_t e = grx::launch_rhs_vertex(p, recon, static_cast<cudaStream_t>(cuda_stream));
+    // the face-once traversal of the LDG kernel with vertex loads; GRX_VARIANT_SIMPLE takes the one-thread-per-cell
+    // cross-check traversal (every face evaluated by both of its cells)
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const cudaError_t e = g_variant.load() == GRX_VARIANT_SIMPLE ? grx::launch_rhs_vertex(p, recon, st)
+                                                                 : grx::launch_rhs_fused_vertex(p, recon, st);
     if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_vertex launch");
     return GRX_OK;
 }

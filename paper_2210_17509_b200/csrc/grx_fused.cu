@@ -16,6 +16,7 @@
 //   * Sources: metric derivatives and the 3+1 source terms per cell, added to the same accumulators.
 // Global loads go through L1/L2 (__ldg); lanes run along x, so every load is a contiguous 256 B row segment.
 #include "grx_launch.h"
+#include "grx_vertex.cuh"
 
 namespace grx {
 
@@ -48,17 +49,23 @@ __device__ __forceinline__ void recon8(const double* __restrict__ prim, long lon
     }
 }
 
-// HLLE flux of the face between cells iL and iR = iL + s from given left/right states.
-template <int D>
+// HLLE flux of the face between cells iL and iR = iL + s from given left/right states.  VERTEX (NEXT-3, reading R31): met
+// is a vertex array and the face metric is the mean of the 4 vertices of the low D-face of cell iR, whose low-corner
+// vertex is vR.
+template <int D, bool VERTEX>
 __device__ __forceinline__ void face8(const double* __restrict__ prim, const double* __restrict__ met, long long nc,
-                                      long long iL, long long iR, const double PL[8], const double PR[8], double gamma,
-                                      double Fh[8], unsigned& nfb) {
+                                      const VStride& vs, long long iL, long long iR, long long vR, const double PL[8],
+                                      const double PR[8], double gamma, double Fh[8], unsigned& nfb) {
     FaceGeom m;
-    m.alp = 0.5 * (ldg(met + iL) + ldg(met + iR));
+    if (VERTEX) {
+        face_geom_vertex<D>(met, vs, vR, m);
+    } else {
+        m.alp = 0.5 * (ldg(met + iL) + ldg(met + iR));
 #pragma unroll
-    for (int a = 0; a < 3; ++a) m.beta[a] = 0.5 * (ldg(met + (1 + a) * nc + iL) + ldg(met + (1 + a) * nc + iR));
+        for (int a = 0; a < 3; ++a) m.beta[a] = 0.5 * (ldg(met + (1 + a) * nc + iL) + ldg(met + (1 + a) * nc + iR));
 #pragma unroll
-    for (int c = 0; c < 6; ++c) m.g[c] = 0.5 * (ldg(met + (4 + c) * nc + iL) + ldg(met + (4 + c) * nc + iR));
+        for (int c = 0; c < 6; ++c) m.g[c] = 0.5 * (ldg(met + (4 + c) * nc + iL) + ldg(met + (4 + c) * nc + iR));
+    }
     face_flux<D>(m, PL, PR, prim + iL, prim + iR, nc, gamma, Fh, nfb);
 }
 
@@ -68,9 +75,9 @@ __device__ __forceinline__ void face8(const double* __restrict__ prim, const dou
 #define GRX_ACC_STORE _Pragma("unroll") for (int q_ = 0; q_ < 8; ++q_) apark[q_ * ((TY + 1) * 32)] = acc[q_];
 constexpr int PARK_SLOTS = 16;   // doubles per thread: z carry q^+[8], running sum[8]
 
-template <int RECON, int TY, int MINB>
+template <int RECON, int TY, int MINB, bool VERTEX>
 __global__ void __launch_bounds__((TY + 1) * 32, MINB)
-rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
+rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg, const VStride vs) {
     extern __shared__ double smem_raw[];
     Exch<TY>& Qb = *reinterpret_cast<Exch<TY>*>(smem_raw);
     Exch<TY>& Fb = *reinterpret_cast<Exch<TY>*>(smem_raw + sizeof(Exch<TY>) / sizeof(double));
@@ -86,12 +93,13 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     const double* __restrict__ prim = p.prim + (long long)box * 8 * p.nc;
-    const double* __restrict__ met = p.met + (long long)box * 10 * p.nc;
-    const double* __restrict__ Kf = p.K + (long long)box * 6 * p.nc;
+    const double* __restrict__ met = p.met + (long long)box * 10 * (VERTEX ? vs.nv : p.nc);
+    const double* __restrict__ Kf = p.K + (long long)box * 6 * (VERTEX ? vs.nv : p.nc);
     double* __restrict__ out = p.out + (long long)box * 8 * p.nc;
     const long long nc = p.nc, sy = p.stride[1], sz = p.stride[2];
     const double gamma = p.gamma;
     const long long cbase = (X0 + p.g) + sy * (Y0 + p.g) + sz * (k0 - 1 + p.g);   // tile origin, plane k0-1
+    const long long vbase = (X0 + p.g) + vs.s[1] * (Y0 + p.g) + vs.s[2] * (k0 - 1 + p.g);   // ... and its low-corner vertex
     unsigned nfb = 0;
     volatile double* apark = smem_raw + 2 * sizeof(Exch<TY>) / sizeof(double) + 8 * (TY + 1) * 32 + threadIdx.x;
 
@@ -99,6 +107,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
         // ------------------------------------------------ regular warp: one cell column per thread
         const bool active = (lane < txe) && (warp < tye);
         long long c = cbase + lane + sy * warp;
+        long long v = vbase + lane + vs.s[1] * warp;      // low-corner vertex of the cell (VERTEX only)
         // q^+ of the previous plane waits in a thread-private shared-memory slot between two z faces (it is
         // needed once per step; parking it frees 16 registers during the x, y and source phases)
         volatile double* zpark = smem_raw + 2 * sizeof(Exch<TY>) / sizeof(double) + threadIdx.x;
@@ -106,8 +115,8 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
         double acc[8];
 #pragma unroll
         for (int q = 0; q < 8; ++q) acc[q] = 0.0;
-        for (int kk = -1; kk <= nk; ++kk, c += sz) {
-            if (tg.pf && active && kk < nk) {
+        for (int kk = -1; kk <= nk; ++kk, c += sz, v += vs.s[2]) {
+            if (!VERTEX && tg.pf && active && kk < nk) {
                 // first touches of this column: metric plane k+2 (z derivative at the end of THIS step), K_ij of
                 // this plane, primitives of plane k+3 (z stencil at the top of the next step)
                 if (tg.pf & 1) {
@@ -134,7 +143,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                     double qpz[8];
 #pragma unroll
                     for (int q = 0; q < 8; ++q) qpz[q] = zpark[q * ZS];
-                    face8<2>(prim, met, nc, c - sz, c, qpz, qm, gamma, Fh, (kk == 0 && k0 > 0) ? dup : nfb);
+                    face8<2, VERTEX>(prim, met, nc, vs, c - sz, c, v, qpz, qm, gamma, Fh, (kk == 0 && k0 > 0) ? dup : nfb);
                     // F/dz is rounded once and used with both signs, so a uniform state cancels exactly
 #pragma unroll
                     for (int q = 0; q < 8; ++q) Fh[q] = __dmul_rn(Fh[q], p.idx[2]);
@@ -164,7 +173,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 double PL[8], Fh[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][warp][lane];
-                face8<0>(prim, met, nc, c - 1, c, PL, qm, gamma, Fh, nfb);
+                face8<0, VERTEX>(prim, met, nc, vs, c - 1, c, v, PL, qm, gamma, Fh, nfb);
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][warp][lane] = Fh[q];
             }
@@ -185,7 +194,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 double PL[8], Fh[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][warp][lane];
-                face8<1>(prim, met, nc, c - sy, c, PL, qm, gamma, Fh, nfb);
+                face8<1, VERTEX>(prim, met, nc, vs, c - sy, c, v, PL, qm, gamma, Fh, nfb);
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][warp][lane] = Fh[q];
             }
@@ -195,7 +204,8 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) acc[q] = fma(Fb.v[q][warp][lane] - Fb.v[q][warp + 1][lane], p.idx[1], acc[q]);
                 double s1, s2, s3, s4;
-                sources_from_global(p, prim, met, Kf, c, s1, s2, s3, s4);
+                if (VERTEX) sources_from_vertices(p, vs, prim, met, Kf, c, v, s1, s2, s3, s4);
+                else sources_from_global(p, prim, met, Kf, c, s1, s2, s3, s4);
                 acc[1] += s1; acc[2] += s2; acc[3] += s3; acc[4] += s4;
                 GRX_ACC_STORE
             }
@@ -214,6 +224,7 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
         unsigned dup = 0;
         for (int kk = 0; kk < nk; ++kk) {
             const long long cp = cbase + sz * (kk + 1);   // tile origin in plane k0+kk
+            const long long vp = vbase + vs.s[2] * (kk + 1);
             double yb_qp[8], yt_qm[8], xr_qm[8];
             long long cxr = 0, cyt = 0;
             if (ycol) {
@@ -238,7 +249,8 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 double PL[8], Fh[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][xrow][txe];
-                face8<0>(prim, met, nc, cxr - 1, cxr, PL, xr_qm, gamma, Fh, count_x ? nfb : dup);
+                face8<0, VERTEX>(prim, met, nc, vs, cxr - 1, cxr, vp + vs.s[1] * xrow + txe, PL, xr_qm, gamma, Fh,
+                                 count_x ? nfb : dup);
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][xrow][txe] = Fh[q];
             }
@@ -252,7 +264,8 @@ rhs_fused_kernel(const __grid_constant__ RhsParams p, const TileGeom tg) {
                 double PL[8], Fh[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) PL[q] = Qb.v[q][tye][lane];
-                face8<1>(prim, met, nc, cyt - sy, cyt, PL, yt_qm, gamma, Fh, count_y ? nfb : dup);
+                face8<1, VERTEX>(prim, met, nc, vs, cyt - sy, cyt, vp + lane + vs.s[1] * tye, PL, yt_qm, gamma, Fh,
+                                 count_y ? nfb : dup);
 #pragma unroll
                 for (int q = 0; q < 8; ++q) Fb.v[q][tye][lane] = Fh[q];
             }
@@ -293,7 +306,7 @@ TileGeom make_tiles(const RhsParams& p, int ty, int slots, double* eff_out = nul
 
 // No cached state: the SM count and the shared-memory opt-in are per device and are queried / set on every launch
 // (both are cheap), so the library works with several devices and from several host threads.
-template <int RECON, int TY, int MINB>
+template <int RECON, int TY, int MINB, bool VERTEX>
 cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
     int dev = 0, sms = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -301,11 +314,11 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return e;
     const size_t smem = 2 * sizeof(Exch<TY>) + PARK_SLOTS * (TY + 1) * 32 * sizeof(double);
-    e = cudaFuncSetAttribute(rhs_fused_kernel<RECON, TY, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    e = cudaFuncSetAttribute(rhs_fused_kernel<RECON, TY, MINB, VERTEX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const TileGeom tg = make_tiles(p, TY, sms * MINB);
     const dim3 grid((unsigned)(tg.ntx * tg.nty * tg.nzc), p.nbox);
-    rhs_fused_kernel<RECON, TY, MINB><<<grid, (TY + 1) * 32, smem, st>>>(p, tg);
+    rhs_fused_kernel<RECON, TY, MINB, VERTEX><<<grid, (TY + 1) * 32, smem, st>>>(p, tg, vstride(p));
     return cudaGetLastError();
 }
 
@@ -313,10 +326,10 @@ cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
 // amortise the taller tile and take the 7-row one (8 warps, 255 registers).
 // tile_nz: the plane count the tile is chosen for -- that of the whole block when p is a z range of it, so that every
 // plane carries the bits of the whole-block call (the two instantiations round differently).
-template <int RECON>
+template <int RECON, bool VERTEX>
 cudaError_t dispatch(const RhsParams& p, int tile_nz, cudaStream_t st) {
-    if (tile_nz < 8) return launch_one<RECON, 7, 1>(p, st);
-    return launch_one<RECON, 11, 1>(p, st);
+    if (tile_nz < 8) return launch_one<RECON, 7, 1, VERTEX>(p, st);
+    return launch_one<RECON, 11, 1, VERTEX>(p, st);
 }
 
 }  // namespace
@@ -329,9 +342,16 @@ double fused_tile_efficiency(const RhsParams& p, int sms) {
 
 cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st, int tile_nz) {
     if (tile_nz <= 0) tile_nz = p.n[2];
-    if (recon == RECON_WENO5) return dispatch<RECON_WENO5>(p, tile_nz, st);
-    if (recon == RECON_MC) return dispatch<RECON_MC>(p, tile_nz, st);
-    return dispatch<RECON_MINMOD>(p, tile_nz, st);
+    if (recon == RECON_WENO5) return dispatch<RECON_WENO5, false>(p, tile_nz, st);
+    if (recon == RECON_MC) return dispatch<RECON_MC, false>(p, tile_nz, st);
+    return dispatch<RECON_MINMOD, false>(p, tile_nz, st);
+}
+
+// NEXT-3: the same kernel with p.met / p.K pointing at vertex arrays (reading R31)
+cudaError_t launch_rhs_fused_vertex(const RhsParams& p, int recon, cudaStream_t st) {
+    if (recon == RECON_WENO5) return dispatch<RECON_WENO5, true>(p, p.n[2], st);
+    if (recon == RECON_MC) return dispatch<RECON_MC, true>(p, p.n[2], st);
+    return dispatch<RECON_MINMOD, true>(p, p.n[2], st);
 }
 
 }  // namespace grx

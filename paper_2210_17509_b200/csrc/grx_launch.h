@@ -11,6 +11,7 @@ namespace grx {
 cudaError_t launch_rhs_simple(const RhsParams& p, int recon, cudaStream_t st);
 // grx_fused.cu: the round-1 kernel (operands through L1), the path for arrays the TMA kernel cannot take
 cudaError_t launch_rhs_fused(const RhsParams& p, int recon, cudaStream_t st, int tile_nz = 0);   // tile_nz: see grx_fused.cu
+cudaError_t launch_rhs_fused_vertex(const RhsParams& p, int recon, cudaStream_t st);   // NEXT-3: p.met, p.K = vertex arrays
 double fused_tile_efficiency(const RhsParams& p, int sms);   // expected fill of the launch geometry, in (0, 1]
 
 // grx_tma.cu: the product kernel (TMA-staged planes, shared-memory z rings); needs even Nx and 16-byte aligned arrays

@@ -7,22 +7,15 @@
 //                        [27 (m(+1/2) - m(-1/2)) - (m(+3/2) - m(-3/2))] / (24 dx) of the transverse 4-vertex means;
 //   tmunu_vertex_kernel  interpolates the 8 primitives to the vertices with the tensor product of (-1, 9, 9, -1)/16
 //                        ("4th-order symmetric 3D interpolation", l.84) and evaluates T^{mu nu} (Eq. 5) there.
-// First correct version: one thread per cell / vertex straight from global memory (every face is evaluated by both of its
-// cells, as in grx_simple.cu); the staged, face-once traversal of grx_tma.cu is what comes next for this centring.
+// rhs_vertex_kernel is the cross-check traversal of this centring (one thread per cell straight from global memory, every face
+// evaluated by both of its cells, as in grx_simple.cu); the product path of grx_valencia_rhs_vertex is the face-once tile
+// traversal rhs_fused_kernel<..., VERTEX> in grx_fused.cu, which shares the vertex loads of grx_vertex.cuh.
 #include "grx_launch.h"
+#include "grx_vertex.cuh"
 
 namespace grx {
 
 namespace {
-
-struct VStride {
-    long long s[3];   // vertex strides: 1, Nx+1, (Nx+1)(Ny+1)
-    long long nv;     // vertices per field
-};
-
-__device__ __forceinline__ double mean4(const double* __restrict__ f, long long v, long long a, long long b) {
-    return 0.25 * ((ldg(f + v) + ldg(f + v + b)) + (ldg(f + v + a) + ldg(f + v + a + b)));
-}
 
 // Face between cell iL and cell iR = iL + s along D; vR = vertex index of the low corner of cell iR.
 template <int D, int RECON>
@@ -43,13 +36,8 @@ __device__ __forceinline__ void face_vertex(const double* __restrict__ prim, con
         recon_cell<RECON>(m1, c0, c1, p2, p3, qm, qp);
         PR[q] = qm;
     }
-    const long long a = vs.s[(D + 1) % 3], b = vs.s[(D + 2) % 3];
     FaceGeom m;
-    m.alp = mean4(metv, vR, a, b);
-#pragma unroll
-    for (int i = 0; i < 3; ++i) m.beta[i] = mean4(metv + (1 + i) * vs.nv, vR, a, b);
-#pragma unroll
-    for (int c = 0; c < 6; ++c) m.g[c] = mean4(metv + (4 + c) * vs.nv, vR, a, b);
+    face_geom_vertex<D>(metv, vs, vR, m);
     face_flux<D>(m, PL, PR, prim + iL, prim + iR, nc, gamma, Fh, nfb);
 }
 
@@ -85,29 +73,8 @@ __global__ void __launch_bounds__(128) rhs_vertex_kernel(const __grid_constant__
     sweep_vertex<0, RECON>(p, vs, prim, metv, c0, v0, i == p.n[0] - 1, acc, nfb);
     sweep_vertex<1, RECON>(p, vs, prim, metv, c0, v0, j == p.n[1] - 1, acc, nfb);
     sweep_vertex<2, RECON>(p, vs, prim, metv, c0, v0, k == p.n[2] - 1, acc, nfb);
-    // sources: centre = mean of 8 vertices, derivatives = staggered 4th-order differences of 4-vertex means
-    double P[8], mc[10], Kc[6], dm[3][10];
-#pragma unroll
-    for (int q = 0; q < 8; ++q) P[q] = ldg(prim + q * p.nc + c0);
-#pragma unroll
-    for (int f = 0; f < 10; ++f) {
-        const double* mv = metv + f * vs.nv;
-        double lo = 0.0, hi = 0.0;
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            const long long sa = vs.s[a], t1 = vs.s[(a + 1) % 3], t2 = vs.s[(a + 2) % 3];
-            const double m_m2 = mean4(mv, v0 - sa, t1, t2), m_m1 = mean4(mv, v0, t1, t2);
-            const double m_p1 = mean4(mv, v0 + sa, t1, t2), m_p2 = mean4(mv, v0 + 2 * sa, t1, t2);
-            dm[a][f] = fma(27.0, m_p1 - m_m1, -(m_p2 - m_m2)) * (p.idx[a] * (1.0 / 24.0));
-            if (a == 0) { lo = m_m1; hi = m_p1; }
-        }
-        mc[f] = 0.5 * (lo + hi);
-    }
-#pragma unroll
-    for (int c = 0; c < 6; ++c)
-        Kc[c] = 0.5 * (mean4(Kv + c * vs.nv, v0, vs.s[1], vs.s[2]) + mean4(Kv + c * vs.nv, v0 + 1, vs.s[1], vs.s[2]));
     double sx, sy, sz, st;
-    sources_point(P, mc, Kc, dm, p.gamma, sx, sy, sz, st);
+    sources_from_vertices(p, vs, prim, metv, Kv, c0, v0, sx, sy, sz, st);
     acc[1] += sx; acc[2] += sy; acc[3] += sz; acc[4] += st;
 #pragma unroll
     for (int c = 0; c < 8; ++c) out[c * p.nc + c0] = acc[c];
@@ -197,15 +164,6 @@ __global__ void __launch_bounds__(128) tmunu_vertex_kernel(const __grid_constant
     tmunu_point(P, m, p.gamma, T10);
 #pragma unroll
     for (int c = 0; c < 10; ++c) T[c * vs.nv + v0] = T10[c];
-}
-
-VStride vstride(const RhsParams& p) {
-    VStride vs;
-    vs.s[0] = 1;
-    vs.s[1] = p.N[0] + 1;
-    vs.s[2] = (long long)(p.N[0] + 1) * (p.N[1] + 1);
-    vs.nv = vs.s[2] * (p.N[2] + 1);
-    return vs;
 }
 
 }  // namespace

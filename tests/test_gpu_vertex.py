@@ -41,8 +41,12 @@ def _vertex_problem(n, nbox=1, seed=0):
     return prim, met_v, K_v, dx
 
 
-@pytest.mark.parametrize("n,nbox", [((20, 12, 9), 2), ((33, 5, 4), 1), ((1, 1, 1), 1), ((130, 3, 2), 1), ((64, 64, 16), 1)])
-def test_vertex_rhs_parity(grx, oracle, n, nbox):
+@pytest.mark.parametrize("variant", ["auto", "simple"])
+@pytest.mark.parametrize("n,nbox", [((20, 12, 9), 2), ((33, 5, 4), 1), ((1, 1, 1), 1), ((130, 3, 2), 1), ((64, 64, 16), 1),
+                                    ((70, 25, 40), 1)])
+def test_vertex_rhs_parity(grx, oracle, n, nbox, variant):
+    """auto = the face-once tile traversal (rhs_fused_kernel with vertex loads: ragged tiles, thin blocks, several z chunks),
+    simple = one thread per cell."""
     import torch
     prim, met_v, K_v, dx = _vertex_problem(n, nbox)
     gamma = 5.0 / 3.0
@@ -53,11 +57,13 @@ def test_vertex_rhs_parity(grx, oracle, n, nbox):
         out = torch.full_like(d[0], -7.25e300)
         cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
         grx.set_fallback_counter(cnt)
+        grx.set_variant(variant)
         try:
             grx.valencia_rhs_vertex(*d, dx, G, recon, gamma, out=out)
             torch.cuda.synchronize()
         finally:
             grx.set_fallback_counter(None)
+            grx.set_variant("auto")
         got = out.cpu().numpy()
         rel = relerr_per_component(got[ii], ref[ii])
         assert np.all(np.isfinite(got[ii])) and rel.max() <= TOL, f"{n}/{recon}: {rel}"
