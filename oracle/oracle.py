@@ -38,6 +38,8 @@ def lib():
         L.oracle_evolve.argtypes = [ip, C.c_int, dp, dp, dp, dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int,
                                     C.c_int, dp]
         L.oracle_evolve.restype = C.c_int
+        L.oracle_evolve_ct.argtypes = L.oracle_evolve.argtypes
+        L.oracle_evolve_ct.restype = C.c_int
         L.oracle_recon_cell.argtypes = [C.c_int, dp, dp, dp]
         L.oracle_recon_cell.restype = None
         L.oracle_state_flux.argtypes = [dp, dp, C.c_int, C.c_double, dp, dp, dp]
@@ -185,17 +187,18 @@ def tmunu_vertices(prim, metric_v, nghost, gamma):
 BC = {"copy": 0, "periodic": 1}
 
 
-def evolve(prim, metric, K, dx, nghost, recon, gamma, dt, nsteps, rk=2, bc="copy"):
-    """Method of lines around the right-hand side (oracle_evolve): returns (prim, cons, nfail) after `nsteps` steps;
-    `prim` must come with filled ghosts and is not modified."""
+def evolve(prim, metric, K, dx, nghost, recon, gamma, dt, nsteps, rk=2, bc="copy", ct=False):
+    """Method of lines around the right-hand side (oracle_evolve; ct=True: oracle_evolve_ct, the calB components of every
+    right-hand side by flux-CT): returns (prim, cons, nfail) after `nsteps` steps; `prim` must come with filled ghosts and
+    is not modified."""
     prim = np.array(prim, dtype=np.float64, order="C", copy=True)
     metric, K = _arr(metric), _arr(K)
     n, nbox = _grid(prim, nghost)
     cons = np.zeros_like(prim)
     dxa = (C.c_double * 3)(*dx)
     r = RECON[recon] if isinstance(recon, str) else int(recon)
-    nfail = lib().oracle_evolve(n, nbox, _p(prim), _p(metric), _p(K), dxa, nghost, r, gamma, dt, int(nsteps), int(rk),
-                                BC[bc], _p(cons))
+    fn = lib().oracle_evolve_ct if ct else lib().oracle_evolve
+    nfail = fn(n, nbox, _p(prim), _p(metric), _p(K), dxa, nghost, r, gamma, dt, int(nsteps), int(rk), BC[bc], _p(cons))
     if nfail < 0:
         raise ValueError("oracle: invalid argument")
     return prim, cons, nfail

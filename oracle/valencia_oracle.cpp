@@ -951,8 +951,13 @@ int oracle_con2prim(const int n[3], int nbox, const double* cons, const double* 
 // con2prim on the interior (step 1 of the paper's RHS evaluation, l.129) and their ghost zones are filled (bc = 0 copy,
 // 1 periodic).  prim (in/out) must come with filled ghosts; cons (out, may be NULL) receives U on the interior (ghosts 0).
 // Returns the number of con2prim failures (>= 0) or -1 for invalid arguments.
-int oracle_evolve(const int n[3], int nbox, double* prim, const double* metric, const double* K, const double dx[3],
-                  int nghost, int recon, double gamma, double dt, int nsteps, int rk, int bc, double* cons) {
+int oracle_face_bfluxes(const int n[3], int nbox, const double* prim, const double* metric, int nghost, int recon,
+                        double gamma, double* FB);
+int oracle_flux_ct(const int n[3], int nbox, const double* FB, const double dx[3], int nghost, double* dB);
+
+// ct = 1: the calB components of every right-hand side are the flux-CT update (NEXT-2, R30) instead of the plain flux difference.
+static int evolve_impl(const int n[3], int nbox, double* prim, const double* metric, const double* K, const double dx[3],
+                       int nghost, int recon, double gamma, double dt, int nsteps, int rk, int bc, double* cons, int ct) {
     if (!n || !prim || !metric || !K || !dx || nbox < 1 || nsteps < 0 || (rk != 2 && rk != 4) || (bc != 0 && bc != 1)) return -1;
     if (!(gamma > 1.0) || nghost < (recon == RECON_WENO5 ? 3 : 2)) return -1;
     Grid G;
@@ -993,7 +998,21 @@ int oracle_evolve(const int n[3], int nbox, double* prim, const double* metric, 
             fill_ghosts_box(G, prim + off, bc);
         }
     };
-    auto rhs = [&]() { return rhs_all<double>(n, nbox, prim, metric, K, dx, nghost, recon, gamma, L.data(), nullptr, nullptr); };
+    std::vector<double> FB, dB;
+    if (ct) { FB.assign(9 * NC * (size_t)nbox, 0.0); dB.assign(3 * NC * (size_t)nbox, 0.0); }
+    auto rhs = [&]() {
+        if (rhs_all<double>(n, nbox, prim, metric, K, dx, nghost, recon, gamma, L.data(), nullptr, nullptr)) return 1;
+        if (!ct) return 0;
+        if (oracle_face_bfluxes(n, nbox, prim, metric, nghost, recon, gamma, FB.data())) return 1;
+        if (oracle_flux_ct(n, nbox, FB.data(), dx, nghost, dB.data())) return 1;
+        for (int bx = 0; bx < nbox; ++bx)
+            for (int c = 0; c < 3; ++c)
+                for (int k = 0; k < G.n[2]; ++k)
+                    for (int j = 0; j < G.n[1]; ++j)
+                        for (int i = 0; i < G.n[0]; ++i)
+                            L[(size_t)bx * 8 * NC + (5 + c) * NC + G.idx(i, j, k)] = dB[(size_t)bx * 3 * NC + c * NC + G.idx(i, j, k)];
+        return 0;
+    };
     for (int s = 0; s < nsteps; ++s) {
         U0 = U;
         if (rk == 2) {
@@ -1031,6 +1050,16 @@ int oracle_evolve(const int n[3], int nbox, double* prim, const double* metric, 
                             cons[o] = U[o];
                         }
     return nfail;
+}
+
+int oracle_evolve(const int n[3], int nbox, double* prim, const double* metric, const double* K, const double dx[3],
+                  int nghost, int recon, double gamma, double dt, int nsteps, int rk, int bc, double* cons) {
+    return evolve_impl(n, nbox, prim, metric, K, dx, nghost, recon, gamma, dt, nsteps, rk, bc, cons, 0);
+}
+
+int oracle_evolve_ct(const int n[3], int nbox, double* prim, const double* metric, const double* K, const double dx[3],
+                     int nghost, int recon, double gamma, double dt, int nsteps, int rk, int bc, double* cons) {
+    return evolve_impl(n, nbox, prim, metric, K, dx, nghost, recon, gamma, dt, nsteps, rk, bc, cons, 1);
 }
 
 // ---- point-level entry points used by the pins (tests/test_oracle_pins*.py) -------------------------
