@@ -203,6 +203,15 @@ int grx_valencia_rhs_vertex(const grx_grid* grid, const double* prim, const doub
 int grx_tmunu_vertices(const grx_grid* grid, const double* prim, const double* metric_v, int nghost, double gamma, double* T,
                        void* cuda_stream);
 
+/* grx_step_rk with constrained transport (NEXT-1 + NEXT-2; the paper's multi-dimensional tests, l.287, l.299): every right-hand
+ * side of every stage is grx_valencia_rhs_ct, so the vertex-centred divergence of calB stays what it was initially, to
+ * rounding.  Arguments as for grx_step_rk; workspace: at least grx_step_ct_workspace_bytes(grid, nghost, rk_order) bytes (the
+ * arrays of grx_step_rk followed by the six face-flux arrays). */
+size_t grx_step_ct_workspace_bytes(const grx_grid* grid, int nghost, int rk_order);
+int grx_step_rk_ct(const grx_grid* grid, double* cons, double* prim, const double* metric, const double* K,
+                   const double dx[3], int nghost, int recon, double gamma, double dt, int rk_order, int bc, int nsteps,
+                   void* workspace, size_t workspace_bytes, unsigned long long* nfail, void* cuda_stream);
+
 /* Debug: if `counter` (DEVICE pointer to one unsigned long long, caller-zeroed) is non-NULL, later
  * grx_valencia_rhs calls of this host thread add to it the number of face sides that took the R5
  * first-order fallback.  NULL switches counting off (the default; counting costs a few atomics). */

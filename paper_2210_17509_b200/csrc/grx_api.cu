@@ -108,6 +108,30 @@ cudaError_t host_streams(cudaStream_t* up, cudaStream_t* dn) {
     return cudaSuccess;
 }
 
+// Right-hand side with constrained transport (NEXT-2): p.fb is set.  The TMA kernel writes the face fluxes of the interior
+// grid lines while it evaluates the right-hand side; the other kernels do not, and then every face is evaluated by the
+// face kernel.  Same kernel choice as grx_valencia_rhs, so that out[0..4] are its bits.
+cudaError_t launch_rhs_ct(grx::RhsParams p, int recon, cudaStream_t st, bool* unsupported) {
+    const int kernel = choose_kernel(p, recon);
+    if (kernel < 0) {
+        if (unsupported) *unsupported = true;
+        return cudaErrorNotSupported;
+    }
+    const bool fused_faces = (kernel == 2);
+    cudaError_t e;
+    if (fused_faces) {
+        e = grx::launch_rhs_tma(p, recon, 7, st);
+    } else {
+        grx::RhsParams q = p;
+        q.fb = nullptr;
+        e = launch_variant(q, recon, st);
+    }
+    p.nfallback = nullptr;   // the faces next to the block are not faces of the right-hand side: not counted
+    if (e == cudaSuccess) e = grx::launch_face_bflux(p, recon, !fused_faces, st);
+    if (e == cudaSuccess) e = grx::launch_flux_ct(p, st);
+    return e;
+}
+
 }  // namespace
 
 extern "C" {
@@ -453,23 +477,9 @@ int grx_valencia_rhs_ct(const grx_grid* grid, const double* prim, const double* 
     p.nfallback = t_fallback_counter;
     p.fb = static_cast<double*>(workspace);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    // The TMA kernel writes the face fluxes of the interior grid lines while it evaluates the right-hand side (p.fb set);
-    // the other kernels do not, and then every face is evaluated by the face kernel.  Same kernel choice as
-    // grx_valencia_rhs, so that out[0..4] are its bits.
-    const int kernel = choose_kernel(p, recon);
-    if (kernel < 0) return fail(GRX_ERR_UNSUPPORTED, "GRX_VARIANT_TMA needs even nx + 2 nghost and 16-byte aligned arrays");
-    const bool fused_faces = (kernel == 2);
-    cudaError_t e;
-    if (fused_faces) {
-        e = grx::launch_rhs_tma(p, recon, 7, st);
-    } else {
-        grx::RhsParams q = p;
-        q.fb = nullptr;
-        e = launch_variant(q, recon, st);
-    }
-    p.nfallback = nullptr;   // the faces next to the block are not faces of the right-hand side: not counted
-    if (e == cudaSuccess) e = grx::launch_face_bflux(p, recon, !fused_faces, st);
-    if (e == cudaSuccess) e = grx::launch_flux_ct(p, st);
+    bool unsupported = false;
+    const cudaError_t e = launch_rhs_ct(p, recon, st, &unsupported);
+    if (unsupported) return fail(GRX_ERR_UNSUPPORTED, "GRX_VARIANT_TMA needs even nx + 2 nghost and 16-byte aligned arrays");
     if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_ct launch");
     return GRX_OK;
 }
@@ -481,9 +491,32 @@ size_t grx_step_workspace_bytes(const grx_grid* grid, int nghost, int rk_order) 
     return (size_t)(rk_order == 2 ? 2 : 3) * 8 * (size_t)p.nc * (size_t)p.nbox * sizeof(double);
 }
 
+size_t grx_step_ct_workspace_bytes(const grx_grid* grid, int nghost, int rk_order) {
+    const size_t a = grx_step_workspace_bytes(grid, nghost, rk_order), b = grx_ct_workspace_bytes(grid, nghost);
+    return (a && b) ? a + b : 0;
+}
+
+static int step_rk_impl(const grx_grid* grid, double* cons, double* prim, const double* metric, const double* K,
+                        const double dx[3], int nghost, int recon, double gamma, double dt, int rk_order, int bc, int nsteps,
+                        void* workspace, size_t workspace_bytes, unsigned long long* nfail, void* cuda_stream, bool ct);
+
 int grx_step_rk(const grx_grid* grid, double* cons, double* prim, const double* metric, const double* K,
                 const double dx[3], int nghost, int recon, double gamma, double dt, int rk_order, int bc, int nsteps,
                 void* workspace, size_t workspace_bytes, unsigned long long* nfail, void* cuda_stream) {
+    return step_rk_impl(grid, cons, prim, metric, K, dx, nghost, recon, gamma, dt, rk_order, bc, nsteps, workspace,
+                        workspace_bytes, nfail, cuda_stream, false);
+}
+
+int grx_step_rk_ct(const grx_grid* grid, double* cons, double* prim, const double* metric, const double* K,
+                   const double dx[3], int nghost, int recon, double gamma, double dt, int rk_order, int bc, int nsteps,
+                   void* workspace, size_t workspace_bytes, unsigned long long* nfail, void* cuda_stream) {
+    return step_rk_impl(grid, cons, prim, metric, K, dx, nghost, recon, gamma, dt, rk_order, bc, nsteps, workspace,
+                        workspace_bytes, nfail, cuda_stream, true);
+}
+
+static int step_rk_impl(const grx_grid* grid, double* cons, double* prim, const double* metric, const double* K,
+                        const double dx[3], int nghost, int recon, double gamma, double dt, int rk_order, int bc, int nsteps,
+                        void* workspace, size_t workspace_bytes, unsigned long long* nfail, void* cuda_stream, bool ct) {
     grx::RhsParams p;
     std::memset(&p, 0, sizeof(p));
     if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
@@ -501,7 +534,8 @@ int grx_step_rk(const grx_grid* grid, double* cons, double* prim, const double* 
         p.idx[a] = 1.0 / dx[a];
     }
     const size_t arr = 8 * (size_t)p.nc * (size_t)p.nbox;
-    if (workspace_bytes < (size_t)(rk_order == 2 ? 2 : 3) * arr * sizeof(double))
+    const size_t nrk = (size_t)(rk_order == 2 ? 2 : 3);
+    if (workspace_bytes < (nrk * arr + (ct ? 6 * (size_t)p.nc * (size_t)p.nbox : 0)) * sizeof(double))
         return fail(GRX_ERR_INVALID_ARG, "workspace too small");
     double* U0 = static_cast<double*>(workspace);
     double* L = U0 + arr;
@@ -509,9 +543,10 @@ int grx_step_rk(const grx_grid* grid, double* cons, double* prim, const double* 
     p.prim = prim; p.met = metric; p.K = K; p.out = L;
     p.gamma = gamma;
     p.nfallback = nullptr;
+    p.fb = ct ? U0 + nrk * arr : nullptr;      // the six face-flux arrays of constrained transport follow the RK arrays
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     cudaError_t e = cudaSuccess;
-    auto rhs = [&]() { return launch_variant(p, recon, st); };
+    auto rhs = [&]() { return ct ? launch_rhs_ct(p, recon, st, nullptr) : launch_variant(p, recon, st); };
     auto stage = [&](double a, const double* Ua, double b, const double* Ub, double h, double* ac, double wdt) {
         cudaError_t r = grx::launch_rk_stage(p, a, Ua, b, Ub, h, L, cons, ac, wdt, prim, nfail, st);
         return r != cudaSuccess ? r : grx::launch_fill_ghosts(p, prim, bc, 7, st);

@@ -18,7 +18,7 @@ RECON = {"minmod": 0, "mc": 1, "weno5": 2}
 VARIANT = {"auto": 0, "simple": 1, "ldg": 2, "tma": 3}
 EXPORTS = (
     "grx_valencia_rhs", "grx_valencia_rhs_host", "grx_host_workspace_bytes", "grx_prim2con", "grx_con2prim", "grx_rk_axpy",
-    "grx_step_rk", "grx_step_workspace_bytes", "grx_valencia_rhs_ct", "grx_ct_workspace_bytes",
+    "grx_step_rk", "grx_step_workspace_bytes", "grx_step_rk_ct", "grx_step_ct_workspace_bytes", "grx_valencia_rhs_ct", "grx_ct_workspace_bytes",
     "grx_valencia_rhs_vertex", "grx_tmunu_vertices", "grx_valencia_rhs_zrange", "grx_halo_z", "grx_halo_z_bytes", "grx_fill_ghosts", "grx_rk_stage", "grx_debug_set_fallback_counter",
     "grx_set_variant", "grx_selftest_math", "grx_dfma_peak_launch", "grx_fp64_issue_probe", "grx_last_error", "grx_version",
     "grx_weno_eps", "grx_v2max",
@@ -55,6 +55,8 @@ def lib():
         L.grx_rk_axpy.argtypes = [gp, i, dbl, vp, dbl, dbl, vp, vp, vp]
         L.grx_step_workspace_bytes.argtypes = [gp, i, i]
         L.grx_step_rk.argtypes = [gp, vp, vp, vp, vp, d3, i, i, dbl, dbl, i, i, i, vp, sz, vp, vp]
+        L.grx_step_rk_ct.argtypes = L.grx_step_rk.argtypes
+        L.grx_step_ct_workspace_bytes.argtypes = [gp, i, i]
         L.grx_ct_workspace_bytes.argtypes = [gp, i]
         L.grx_valencia_rhs_ct.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, vp, sz, vp]
         L.grx_valencia_rhs_zrange.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, i, i, vp]
@@ -73,6 +75,7 @@ def lib():
             getattr(L, name).restype = C.c_int
         L.grx_host_workspace_bytes.restype = sz
         L.grx_step_workspace_bytes.restype = sz
+        L.grx_step_ct_workspace_bytes.restype = sz
         L.grx_ct_workspace_bytes.restype = sz
         L.grx_halo_z_bytes.restype = sz
         L.grx_last_error.restype = C.c_char_p
@@ -217,18 +220,22 @@ def step_workspace_bytes(shape, nghost, rk):
 
 
 def step_rk(cons, prim, metric, K, dx, nghost, recon, gamma, dt, nsteps, rk=2, bc="copy", workspace=None, nfail=None,
-            stream=None):
-    """grx_step_rk: `nsteps` device-resident method-of-lines steps (in place in cons and prim).  `workspace`: CUDA tensor
-    of at least step_workspace_bytes(...) bytes (allocated if not given)."""
+            stream=None, ct=False):
+    """grx_step_rk (ct=True: grx_step_rk_ct, constrained transport in every stage): `nsteps` device-resident method-of-lines
+    steps (in place in cons and prim).  `workspace`: CUDA tensor of at least step_workspace_bytes(...) bytes (allocated if
+    not given)."""
     import torch
     g = _grid(prim, nghost)
     need = step_workspace_bytes(prim.shape, nghost, rk)
+    if ct:
+        need = lib().grx_step_ct_workspace_bytes(C.byref(g), int(nghost), int(rk))
     if workspace is None:
         workspace = torch.empty(need // 8, dtype=torch.float64, device=prim.device)
     r = RECON[recon] if isinstance(recon, str) else int(recon)
     dxa = (C.c_double * 3)(*[float(v) for v in dx])
     nf = C.c_void_p(nfail.data_ptr()) if nfail is not None else C.c_void_p(0)
-    _check(lib().grx_step_rk(C.byref(g), _dev(cons, 8), _dev(prim, 8), _dev(metric, 10), _dev(K, 6), dxa, int(nghost), r,
+    fn = lib().grx_step_rk_ct if ct else lib().grx_step_rk
+    _check(fn(C.byref(g), _dev(cons, 8), _dev(prim, 8), _dev(metric, 10), _dev(K, 6), dxa, int(nghost), r,
                              float(gamma), float(dt), int(rk), BC[bc] if isinstance(bc, str) else int(bc), int(nsteps),
                              C.c_void_p(workspace.data_ptr()), workspace.numel() * workspace.element_size(), nf,
                              _stream(stream)))

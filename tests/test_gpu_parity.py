@@ -431,10 +431,12 @@ def test_balsara1_rk2_20_steps_gpu_vs_oracle(grx, oracle):
     assert np.abs(y.cpu().numpy()[ii] - expect).max() <= 1e-14 * np.abs(expect).max()
 
 
-@pytest.mark.parametrize("case", ["balsara1-rk2-copy", "balsara1-rk4-copy", "wave-rk4-periodic", "gen-rk2-periodic"])
+@pytest.mark.parametrize("case", ["balsara1-rk2-copy", "balsara1-rk4-copy", "wave-rk4-periodic", "gen-rk2-periodic",
+                                  "wave-rk2-periodic-ct", "gen-rk4-periodic-ct", "balsara1-rk2-copy-ct"])
 def test_device_resident_steps_vs_oracle_loop(grx, oracle, case):
     """NEXT-1: N method-of-lines steps entirely on the device (grx_step_rk: RHS, stage update fused with con2prim, ghost
-    fill; no host round trip) against the same loop of the oracle (oracle_evolve): 1e-10 max|U| per component (R22)."""
+    fill; no host round trip) against the same loop of the oracle (oracle_evolve): 1e-10 max|U| per component (R22).
+    "-ct": grx_step_rk_ct against oracle_evolve_ct (constrained transport in every stage, NEXT-2)."""
     import torch
     from test_oracle_evolve import _periodic_wave
     if case.startswith("balsara1"):
@@ -445,6 +447,7 @@ def test_device_resident_steps_vs_oracle_loop(grx, oracle, case):
         prob, recon, nsteps, cfl = inputs.general_metric_box(n=(20, 12, 10), seed=9, nbox=2), "weno5", 4, 0.2
     rk = 4 if "rk4" in case else 2
     bc = "periodic" if "periodic" in case else "copy"
+    ct = case.endswith("-ct")
     dt = cfl * min(prob.dx)
     prim0 = prob.prim.copy()
     if not case.startswith("wave"):
@@ -459,19 +462,47 @@ def test_device_resident_steps_vs_oracle_loop(grx, oracle, case):
             kk = np.arange(-g, prob.n[2] + g) % prob.n[2] + g
             prim0 = np.ascontiguousarray(prim0[:, :, kk][:, :, :, jj][:, :, :, :, ii])
     p_ref, U_ref, nf_ref = oracle.evolve(prim0, prob.metric, prob.K, prob.dx, prob.nghost, recon, prob.gamma, dt, nsteps,
-                                         rk=rk, bc=bc)
+                                         rk=rk, bc=bc, ct=ct)
     assert nf_ref == 0
     prim = torch.from_numpy(prim0).cuda()
     met, K = torch.from_numpy(prob.metric).cuda(), torch.from_numpy(prob.K).cuda()
     cons = grx.prim2con(prim, met, prob.nghost, prob.gamma)
     nfail = torch.zeros(1, dtype=torch.int64, device="cuda")
-    grx.step_rk(cons, prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, dt, nsteps, rk=rk, bc=bc, nfail=nfail)
+    grx.step_rk(cons, prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, dt, nsteps, rk=rk, bc=bc, nfail=nfail, ct=ct)
     torch.cuda.synchronize()
     assert int(nfail.item()) == 0
     ii = prob.interior
     assert relerr_per_component(cons.cpu().numpy()[ii], U_ref[ii]).max() < 1e-10
     # primitives incl. their ghost zones follow
     assert np.abs(prim.cpu().numpy() - p_ref).max() < 1e-9 * np.abs(p_ref).max()
+
+
+def test_steps_with_constrained_transport_keep_the_vertex_divergence(grx):
+    """grx_step_rk_ct on a periodic multi-tile block whose field is not solenoidal: the vertex-centred divergence of calB
+    after 5 RK2 steps is the initial one to rounding; without CT it is not."""
+    import torch
+    from test_oracle_ct import _vertex_divergence
+    prim_h, met_h, K_h, dx, gamma = inputs._smooth_box((40, 18, 12), 3, inputs.NGHOST)
+    g = inputs.NGHOST
+    prim = torch.from_numpy(prim_h[None].copy()).cuda()
+    met = torch.from_numpy(np.ascontiguousarray(np.broadcast_to(inputs.by_name("c1").metric[:, :, :1, :1, :1], (1, 10) + prim_h.shape[1:]))).cuda()
+    K = torch.zeros((1, 6) + prim_h.shape[1:], dtype=torch.float64, device="cuda")
+    grx.fill_ghosts(prim, g, "periodic", 7)
+    ii = (slice(None), slice(None), slice(g, -g), slice(g, -g), slice(g, -g))
+    res = {}
+    for ct in (True, False):
+        p = prim.clone()
+        cons = grx.prim2con(p, met, g, gamma)
+        if "U0" not in res:
+            res["U0"] = cons[ii].cpu().numpy()
+        grx.step_rk(cons, p, met, K, dx, g, "weno5", gamma, 0.2 * min(dx), 5, rk=2, bc="periodic", ct=ct)
+        torch.cuda.synchronize()
+        res[ct] = cons[ii].cpu().numpy()
+    d0 = _vertex_divergence(res["U0"][0, 5:8], dx)
+    scale = np.abs(res["U0"][0, 5:8]).max() / min(dx)
+    assert np.abs(d0).max() > 1e-2 * scale
+    assert np.abs(_vertex_divergence(res[True][0, 5:8], dx) - d0).max() < 1e-12 * scale
+    assert np.abs(_vertex_divergence(res[False][0, 5:8], dx) - d0).max() > 1e-6 * scale
 
 
 def test_selftest_math_accuracy(grx):
