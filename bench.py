@@ -279,29 +279,30 @@ def time_rhs(grx, torch, prob, dev, recon, steps, warmup, stream):
     return e0.elapsed_time(e1) * 1e-3, out
 
 
-def time_zone_cycles(grx, torch, prob, dev, recon, stream, nsteps=5):
+def time_zone_cycles(grx, torch, prob, dev, recon, stream, nsteps=5, ct=False):
     """zone-cycles/s = steps x cells / time of grx_step_rk: SSP-RK2, periodic ghost fill, every stage =
     RHS + update fused with con2prim + ghost fill, all on the device."""
     prim0, met, K = dev
     prim = prim0.clone()
     grx_bc = "periodic"
     cons = grx.prim2con(prim, met, prob.nghost, prob.gamma)
-    ws = torch.empty(grx.step_workspace_bytes(prim.shape, prob.nghost, 2) // 8, dtype=torch.float64, device="cuda")
+    ws_bytes = grx.step_workspace_bytes(prim.shape, prob.nghost, 2) + (grx.ct_workspace_bytes(prim.shape, prob.nghost) if ct else 0)
+    ws = torch.empty(ws_bytes // 8, dtype=torch.float64, device="cuda")
     nfail = torch.zeros(1, dtype=torch.int64, device="cuda")
     dt = 0.2 * min(prob.dx)
     grx.step_rk(cons, prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, dt, 1, rk=2, bc=grx_bc, workspace=ws, nfail=nfail,
-                stream=stream)      # warm-up step; also makes the ghosts periodic
+                stream=stream, ct=ct)      # warm-up step; also makes the ghosts periodic
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     stream.synchronize()
     e0.record(stream)
     grx.step_rk(cons, prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, dt, nsteps, rk=2, bc=grx_bc, workspace=ws,
-                nfail=nfail, stream=stream)
+                nfail=nfail, stream=stream, ct=ct)
     e1.record(stream)
     stream.synchronize()
     t = e0.elapsed_time(e1) * 1e-3
     ok = bool(torch.isfinite(cons[prob.interior]).all().item())
     return {"value": prob.cells * nsteps / t, "unit": "zone-cycles/s", "steps": nsteps, "ms_per_step": 1e3 * t / nsteps,
-            "scheme": f"SSP-RK2, {recon}+HLLE, Gamma-law con2prim, periodic ghosts, static metric; {prob.name}",
+            "scheme": f"SSP-RK2, {recon}+HLLE{' + flux-CT' if ct else ''}, Gamma-law con2prim, periodic ghosts, static metric; {prob.name}",
             "con2prim_failures": int(nfail.item()), "finite": ok,
             "paper_context": "setupA 0.47e8 zone-cycles/s at 240^3 on one V100 (PAPER.md l.341): other hardware, context only"}
 
@@ -574,6 +575,7 @@ def run_ours(args):
     if not args.no_sweep:
         zone_cycles = time_zone_cycles(grx, torch, prob, dev, recon, stream)
         ct = time_ct(grx, torch, prob, dev, recon, stream)
+        ct["zone_cycles"] = time_zone_cycles(grx, torch, prob, dev, recon, stream, ct=True)
         vertex = time_vertex(grx, torch, prob, dev, recon, stream)
 
     line = {
