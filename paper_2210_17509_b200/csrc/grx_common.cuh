@@ -113,7 +113,7 @@ __device__ __forceinline__ void face_geom_load(const double* __restrict__ mL, in
 // HLLE flux (times `scale` = 1/dx_d) of the face between the cell at (pL, mL) and the next one along stride s.
 template <int D>
 __device__ __forceinline__ void face8s(const double* __restrict__ pL, const double* __restrict__ mL, int nc, int s,
-                                       const double PL[8], const double PR[8], double gamma, double scale,
+                                       double PL[8], double PR[8], double gamma, double scale,
                                        double Fh[8], unsigned& nfb) {
     FaceGeom m;
     face_geom_load(mL, nc, s, m);

@@ -54,8 +54,8 @@ __device__ __forceinline__ void recon8(const double* __restrict__ prim, long lon
 // vertex is vR.
 template <int D, bool VERTEX>
 __device__ __forceinline__ void face8(const double* __restrict__ prim, const double* __restrict__ met, long long nc,
-                                      const VStride& vs, long long iL, long long iR, long long vR, const double PL[8],
-                                      const double PR[8], double gamma, double Fh[8], unsigned& nfb) {
+                                      const VStride& vs, long long iL, long long iR, long long vR, double PL[8],
+                                      double PR[8], double gamma, double Fh[8], unsigned& nfb) {
     FaceGeom m;
     if (VERTEX) {
         face_geom_vertex<D>(met, vs, vR, m);

@@ -148,29 +148,31 @@ GRX_HD void face_geom_complete(FaceGeom& m) {
 }
 
 // ---- a3-a5: one side of a face: admissibility, conserved state, flux, fast speeds -------------------------
-// P: reconstructed primitives of this side; cen[q * nc]: centre values of its donor cell, read only if the
-// side takes the first-order fallback (R5).
+// P: reconstructed primitives of this side (replaced in place by the donor cell's centre values cen[q * nc] if the side
+// takes the first-order fallback, R5).
 // Returns U (Eqs. 6-9, l.88-94) and F^D (Eq. 12, l.108), both WITHOUT their common factor sqrt(gamma), and the two
 // characteristic speeds (R8).
 template <int D>
-GRX_HD void side_state(const double Pin[8], const double* __restrict__ cen, long long nc, const FaceGeom& m,
+GRX_HD void side_state(double P[8], const double* __restrict__ cen, long long nc, const FaceGeom& m,
                        double gamma, double U[8], double F[8], double& lam_m, double& lam_p, unsigned& nfallback) {
-    double rho = Pin[0], vx = Pin[1], vy = Pin[2], vz = Pin[3], eps = Pin[4];
-    double Bx = Pin[5], By = Pin[6], Bz = Pin[7];
+    // P is the caller's array and is overwritten IN PLACE by the fallback (it is dead after the face): copying it into
+    // conditionally reassigned locals cost 16 register moves per side on the common path.
     const double gxx = m.g[0], gxy = m.g[1], gxz = m.g[2], gyy = m.g[3], gyz = m.g[4], gzz = m.g[5];
-    double vlx = fma(gxx, vx, fma(gxy, vy, gxz * vz));      // v_i = gamma_ij v^j
-    double vly = fma(gxy, vx, fma(gyy, vy, gyz * vz));
-    double vlz = fma(gxz, vx, fma(gyz, vy, gzz * vz));
-    double v2 = fma(vlx, vx, fma(vly, vy, vlz * vz));
-    if (!(rho > 0.0 && eps > 0.0 && v2 < V2MAX)) {          // R5; NaN fails the test
-        rho = cen[0]; vx = cen[nc]; vy = cen[2 * nc]; vz = cen[3 * nc]; eps = cen[4 * nc];
-        Bx = cen[5 * nc]; By = cen[6 * nc]; Bz = cen[7 * nc];
-        vlx = fma(gxx, vx, fma(gxy, vy, gxz * vz));
-        vly = fma(gxy, vx, fma(gyy, vy, gyz * vz));
-        vlz = fma(gxz, vx, fma(gyz, vy, gzz * vz));
-        v2 = fma(vlx, vx, fma(vly, vy, vlz * vz));
+    double vlx = fma(gxx, P[1], fma(gxy, P[2], gxz * P[3]));      // v_i = gamma_ij v^j
+    double vly = fma(gxy, P[1], fma(gyy, P[2], gyz * P[3]));
+    double vlz = fma(gxz, P[1], fma(gyz, P[2], gzz * P[3]));
+    double v2 = fma(vlx, P[1], fma(vly, P[2], vlz * P[3]));
+    if (!(P[0] > 0.0 && P[4] > 0.0 && v2 < V2MAX)) {          // R5; NaN fails the test
+#pragma unroll
+        for (int q = 0; q < 8; ++q) P[q] = cen[q * nc];
+        vlx = fma(gxx, P[1], fma(gxy, P[2], gxz * P[3]));
+        vly = fma(gxy, P[1], fma(gyy, P[2], gyz * P[3]));
+        vlz = fma(gxz, P[1], fma(gyz, P[2], gzz * P[3]));
+        v2 = fma(vlx, P[1], fma(vly, P[2], vlz * P[3]));
         ++nfallback;
     }
+    const double rho = P[0], vx = P[1], vy = P[2], vz = P[3], eps = P[4];
+    const double Bx = P[5], By = P[6], Bz = P[7];
     const double iW2 = 1.0 - v2;                             // 1/W^2
     const double W = rsqrt(iW2);                             // l.98
     const double iW = W * iW2;
@@ -240,7 +242,7 @@ GRX_HD void side_state(const double Pin[8], const double* __restrict__ cen, long
 // ---- a6: HLLE flux of one face (l.131; R9) -----------------------------------------------------------------
 // m holds the averaged alp, beta, g on entry; cenL/cenR point at field 0 of the two donor cells (field stride nc).
 template <int D>
-GRX_HD void face_flux(FaceGeom& m, const double PL[8], const double PR[8], const double* __restrict__ cenL,
+GRX_HD void face_flux(FaceGeom& m, double PL[8], double PR[8], const double* __restrict__ cenL,
                       const double* __restrict__ cenR, long long nc, double gamma, double Fh[8], unsigned& nfallback,
                       double scale = 1.0) {
     face_geom_complete<D>(m);
