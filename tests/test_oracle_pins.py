@@ -619,3 +619,39 @@ def test_config2_fallback_count(oracle):
     assert nfb == 64
     _, nfb = oracle.valencia_rhs(prob.prim, prob.metric, prob.K, prob.dx, 3, "minmod", prob.gamma)
     assert nfb == 0
+
+
+def test_r5_admissibility_uses_the_face_metric(oracle):
+    """R5 on a non-flat metric: v^2 = gamma_ij v^i v^j with the FACE metric decides, not the coordinate components.
+    (a) gamma_xx = 4, v^x = 0.6: v^2 = 1.44 -> the side falls back to its donor cell, so the face flux is exactly the one
+        computed from the donor's centre values; the same state is admissible (and gives another flux) on the flat metric.
+    (b) gamma_xx = 0.25, v^x = 1.5: v^2 = 0.5625 -> admissible although the coordinate velocity exceeds 1: the flux is finite
+        and is NOT the fallback's.
+    (c) rho <= 0, eps <= 0 and NaN fail the test too."""
+    gamma = 5.0 / 3.0
+    CL = np.array([1.0, 0.1, 0.05, -0.02, 0.8, 0.3, 0.2, -0.1])
+    CR = np.array([0.9, 0.12, 0.02, 0.01, 0.7, 0.3, 0.25, -0.05])
+    flat = np.array([1.0, 0, 0, 0, 1, 0, 0, 1, 0, 1.0])
+    g4 = flat.copy(); g4[4] = 4.0
+    gq = flat.copy(); gq[4] = 0.25
+    PL = CL.copy(); PL[1] = 0.6
+    for d in range(3):
+        # (a)
+        assert np.array_equal(oracle.face_flux(PL, CR, CL, CR, g4, d, gamma), oracle.face_flux(CL, CR, CL, CR, g4, d, gamma))
+        assert not np.array_equal(oracle.face_flux(PL, CR, CL, CR, flat, d, gamma), oracle.face_flux(CL, CR, CL, CR, flat, d, gamma))
+        # the right side is checked independently of the left one
+        PR = CR.copy(); PR[1] = -0.6
+        assert np.array_equal(oracle.face_flux(CL, PR, CL, CR, g4, d, gamma), oracle.face_flux(CL, CR, CL, CR, g4, d, gamma))
+        # (b)
+        fast = CL.copy(); fast[1] = 1.5
+        F = oracle.face_flux(fast, CR, CL, CR, gq, d, gamma)
+        assert np.all(np.isfinite(F)) and not np.array_equal(F, oracle.face_flux(CL, CR, CL, CR, gq, d, gamma))
+        # (c)
+        for q, bad in ((0, 0.0), (0, -1.0), (4, 0.0), (4, -0.3), (2, np.nan)):
+            P = CL.copy(); P[q] = bad
+            assert np.array_equal(oracle.face_flux(P, CR, CL, CR, flat, d, gamma), oracle.face_flux(CL, CR, CL, CR, flat, d, gamma))
+    # the bound itself: v^2 just below / at 1 - 1e-4 (V2MAX)
+    for v, falls in ((np.sqrt(oracle.v2max()) * (1 - 1e-12), False), (np.sqrt(oracle.v2max()) * (1 + 1e-12), True)):
+        P = CL.copy(); P[1:4] = (v, 0.0, 0.0)
+        same = np.array_equal(oracle.face_flux(P, CR, CL, CR, flat, 0, gamma), oracle.face_flux(CL, CR, CL, CR, flat, 0, gamma))
+        assert same == falls
