@@ -89,13 +89,13 @@ __device__ __forceinline__ void tmunu_point(const double P[8], const double met[
     const double gxx = met[4], gxy = met[5], gxz = met[6], gyy = met[7], gyz = met[8], gzz = met[9];
     const double cof[6] = {fma(gyy, gzz, -gyz * gyz), fma(gxz, gyz, -gxy * gzz), fma(gxy, gyz, -gxz * gyy),
                            fma(gxx, gzz, -gxz * gxz), fma(gxy, gxz, -gxx * gyz), fma(gxx, gyy, -gxy * gxy)};
-    const double idet = 1.0 / fma(gxx, cof[0], fma(gxy, cof[1], gxz * cof[2]));
+    const double idet = rcp(fma(gxx, cof[0], fma(gxy, cof[1], gxz * cof[2])));
     const double vl[3] = {fma(gxx, v[0], fma(gxy, v[1], gxz * v[2])), fma(gxy, v[0], fma(gyy, v[1], gyz * v[2])),
                           fma(gxz, v[0], fma(gyz, v[1], gzz * v[2]))};
     const double Bl[3] = {fma(gxx, B[0], fma(gxy, B[1], gxz * B[2])), fma(gxy, B[0], fma(gyy, B[1], gyz * B[2])),
                           fma(gxz, B[0], fma(gyz, B[1], gzz * B[2]))};
     const double v2 = fma(vl[0], v[0], fma(vl[1], v[1], vl[2] * v[2]));
-    const double iW2 = 1.0 - v2, W = 1.0 / sqrt(iW2), ia = 1.0 / alp;
+    const double iW2 = 1.0 - v2, W = rsqrt(iW2), ia = rcp(alp);
     const double Bv = fma(Bl[0], v[0], fma(Bl[1], v[1], Bl[2] * v[2]));
     const double B2 = fma(Bl[0], B[0], fma(Bl[1], B[1], Bl[2] * B[2]));
     const double ab0 = W * Bv;                                    // alpha b^0
@@ -126,44 +126,54 @@ __device__ __forceinline__ void tmunu_point(const double P[8], const double met[
         }
 }
 
+// One thread per vertex COLUMN (i, j) of a z chunk, marching along z: each step interpolates the 8 primitives of one cell
+// plane to the column's (x, y) position (4 x 4 cells, symmetric pairs first), keeps the last four planes' values in
+// registers and combines them along z -- 128 loads per vertex instead of 512, all of them rows that neighbouring lanes
+// share through L1.  T^{mu nu} is then evaluated with the vertex's own metric sample.
+constexpr int TMUNU_ZCHUNK = 64;
 __global__ void __launch_bounds__(128) tmunu_vertex_kernel(const __grid_constant__ RhsParams p, const VStride vs, double* Tout) {
     const int nxb = (p.n[0] + 1 + 127) / 128;
     const int i = (blockIdx.x % nxb) * 128 + threadIdx.x;
-    const int row = blockIdx.x / nxb;
-    const int j = row % (p.n[1] + 1), k = row / (p.n[1] + 1);
-    const int box = blockIdx.y;
+    const int j = blockIdx.x / nxb;
+    const int k0 = blockIdx.y * TMUNU_ZCHUNK, k1 = min(k0 + TMUNU_ZCHUNK, p.n[2] + 1);     // vertices k0 .. k1-1
+    const int box = blockIdx.z;
     if (i > p.n[0]) return;
     const double* prim = p.prim + (long long)box * 8 * p.nc;
     const double* metv = p.met + (long long)box * 10 * vs.nv;
     double* T = Tout + (long long)box * 10 * vs.nv;
-    // the 4 x 4 x 4 cells around the vertex start at cell (i-2, j-2, k-2)
-    const long long c0 = (i - 2 + p.g) + p.stride[1] * (j - 2 + p.g) + p.stride[2] * (k - 2 + p.g);
-    const long long v0 = (i + p.g) + vs.s[1] * (j + p.g) + vs.s[2] * (k + p.g);
-    const double w[4] = {-1.0 / 16.0, 9.0 / 16.0, 9.0 / 16.0, -1.0 / 16.0};
-    double P[8];
+    // the 4 x 4 cells around the column start at cell (i-2, j-2); vertex k needs the cell planes k-2 .. k+1
+    long long c = (i - 2 + p.g) + p.stride[1] * (j - 2 + p.g) + p.stride[2] * (k0 - 2 + p.g);
+    long long v = (i + p.g) + vs.s[1] * (j + p.g) + vs.s[2] * (k0 + p.g);
+    const double w9 = 9.0 / 16.0, w1 = -1.0 / 16.0;
+    double r0[8], r1[8], r2[8], r3[8];   // in-plane interpolants of the last four cell planes, oldest first
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
-        const double* f = prim + q * p.nc + c0;
-        double sz_ = 0.0;
+    for (int q = 0; q < 8; ++q) r0[q] = r1[q] = r2[q] = r3[q] = 0.0;
+    for (int kz = k0 - 2; kz <= k1; ++kz, c += p.stride[2]) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            double sy_ = 0.0;
+        for (int q = 0; q < 8; ++q) {
+            const double* f = prim + q * p.nc + c;
+            double h[4];
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
-                const double* r = f + c * p.stride[2] + b * p.stride[1];
-                // symmetric pairs first: (f1 + f2) 9/16 - (f0 + f3)/16
-                sy_ = fma(w[b], fma(9.0 / 16.0, ldg(r + 1) + ldg(r + 2), (-1.0 / 16.0) * (ldg(r) + ldg(r + 3))), sy_);
+                const double* r = f + b * p.stride[1];
+                h[b] = fma(w9, ldg(r + 1) + ldg(r + 2), w1 * (ldg(r) + ldg(r + 3)));
             }
-            sz_ = fma(w[c], sy_, sz_);
+            r0[q] = r1[q]; r1[q] = r2[q]; r2[q] = r3[q];
+            r3[q] = fma(w9, h[1] + h[2], w1 * (h[0] + h[3]));
         }
-        P[q] = sz_;
+        const int k = kz - 1;            // the vertex whose four planes are complete now
+        if (k >= k0) {
+            double P[8], m[10], T10[10];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) P[q] = fma(w9, r1[q] + r2[q], w1 * (r0[q] + r3[q]));
+#pragma unroll
+            for (int f = 0; f < 10; ++f) m[f] = ldg(metv + f * vs.nv + v);
+            tmunu_point(P, m, p.gamma, T10);
+#pragma unroll
+            for (int cc = 0; cc < 10; ++cc) T[cc * vs.nv + v] = T10[cc];
+            v += vs.s[2];
+        }
     }
-    double m[10], T10[10];
-#pragma unroll
-    for (int f = 0; f < 10; ++f) m[f] = ldg(metv + f * vs.nv + v0);
-    tmunu_point(P, m, p.gamma, T10);
-#pragma unroll
-    for (int c = 0; c < 10; ++c) T[c * vs.nv + v0] = T10[c];
 }
 
 }  // namespace
@@ -178,7 +188,8 @@ cudaError_t launch_rhs_vertex(const RhsParams& p, int recon, cudaStream_t st) {
 }
 
 cudaError_t launch_tmunu_vertex(const RhsParams& p, double* T, cudaStream_t st) {
-    const dim3 grid((unsigned)((p.n[0] + 1 + 127) / 128) * (unsigned)(p.n[1] + 1) * (unsigned)(p.n[2] + 1), p.nbox);
+    const dim3 grid((unsigned)((p.n[0] + 1 + 127) / 128) * (unsigned)(p.n[1] + 1),
+                    (unsigned)((p.n[2] + 1 + TMUNU_ZCHUNK - 1) / TMUNU_ZCHUNK), p.nbox);
     tmunu_vertex_kernel<<<grid, 128, 0, st>>>(p, vstride(p), T);
     return cudaGetLastError();
 }
