@@ -556,6 +556,8 @@ def run_ours(args):
         if cap.get("fp64_inst_per_cell"):
             # one executed FP64 instruction = one lane-slot of the pipe whatever it does (an FMA counts 2 flops)
             roofline["frac_executed_slots"] = cap["fp64_inst_per_cell"] * cells / t_launch / (148 * 64 * 1.965e9)
+    elif cap is None:
+        roofline["ncu"] = {"csrc_sha": sha, "note": "no ncu capture for this workload / reconstruction / variant"}
     else:
         roofline["ncu"] = {"csrc_sha": sha, "note": "no ncu capture for this state of csrc/ (captured at %s)" % NCU_CAPTURE["csrc_sha"]}
 
