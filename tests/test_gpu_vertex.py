@@ -87,7 +87,7 @@ def test_vertex_rhs_linear_metric_equals_cell_centred_kernel(grx):
     assert relerr_per_component(b[ii].cpu().numpy(), a[ii].cpu().numpy()).max() < 1e-12
 
 
-@pytest.mark.parametrize("n,nbox", [((20, 12, 9), 2), ((1, 1, 1), 1), ((130, 6, 5), 1)])
+@pytest.mark.parametrize("n,nbox", [((20, 12, 9), 2), ((1, 1, 1), 1), ((130, 6, 5), 1), ((10, 6, 135), 1)])
 def test_tmunu_vertices_parity(grx, oracle, n, nbox):
     import torch
     prim, met_v, _, dx = _vertex_problem(n, nbox)
