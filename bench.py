@@ -190,6 +190,12 @@ def time_oracle(prob, recon, budget_s, reps=1):
     return cells / best, best, n1, orc.num_threads()
 
 
+def workload_string(prob, recon):
+    """The same text in both arms, so that the driver sees one config."""
+    return (f"{prob.name} per GPU, {recon}+HLLE, Gamma-law EOS, perturbed conformally flat metric + shift + K_ij, "
+            f"{prob.nghost} ghosts; one right-hand-side evaluation per step")
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -221,8 +227,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{prob.name}, {args.recon}+HLLE, Gamma-law, general metric + K_ij; oracle on host cores",
-                   "l2": "n/a (CPU)"},
+        "config": {"workload": workload_string(prob, args.recon), "l2": "n/a (CPU)", "arm": "oracle on host cores, bounded sample"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -584,8 +589,7 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{prob.name} per GPU, {recon}+HLLE, Gamma-law EOS, perturbed conformally flat metric "
-                               f"+ shift + K_ij, {g} ghosts; one grx_valencia_rhs call per step",
+        "config": {"workload": workload_string(prob, recon), "arm": "one grx_valencia_rhs call per step",
                    "l2": "inputs 4.6 GB >> 126 MB L2, no flush", "variant": args.variant,
                    "parallelism": f"blocks x{world}, no collective"},
         "clocks": clocks,
