@@ -169,7 +169,7 @@ int grx_valencia_rhs_ct(const grx_grid* grid, const double* prim, const double* 
  *   plane and can run while those are in flight; [0, g) and [nz - g, nz) follow when they have arrived.
  * grx_halo_z: pack (unpack = 0) the nghost lowest (side 0) or highest (side 1) INTERIOR planes of the 8 primitive fields into
  *   buf[nbox][8][nghost][Ny][Nx], or unpack (unpack = 1) buf into the low (side 0) / high (side 1) z GHOST planes.  Planes
- *   travel with their x and y ghost cells (fill those first).  buf: DEVICE, grx_halo_z_bytes(grid, nghost) bytes.
+ *   travel with their x and y ghost cells (fill those first).  buf: DEVICE, grx_halo_z_bytes(grid, nghost) bytes; nbox <= 8191.
  * grx_fill_ghosts: the ghost fill of grx_step_rk as a call of its own; dirs = mask of the directions filled here (bit 0 = x,
  *   1 = y, 2 = z): a z-slab rank fills x and y (dirs = 3) and receives z.
  * grx_rk_stage: the stage update of grx_step_rk as a call of its own: Uout = a Ua + b (Ub + h L) on the interior cells,

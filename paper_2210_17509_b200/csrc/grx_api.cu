@@ -398,6 +398,7 @@ int grx_halo_z(const grx_grid* grid, double* prim, int nghost, int side, int unp
     if (!prim || !buf) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
     if (side != 0 && side != 1) return fail(GRX_ERR_INVALID_ARG, "side must be 0 (low) or 1 (high)");
     if (p.n[2] < p.g) return fail(GRX_ERR_INVALID_ARG, "a slab must have at least nghost planes");
+    if (p.nbox > 8191) return fail(GRX_ERR_INVALID_ARG, "grx_halo_z takes at most 8191 boxes per call");
     const cudaError_t e = grx::launch_halo_z(p, prim, buf, side, unpack != 0, static_cast<cudaStream_t>(cuda_stream));
     if (e != cudaSuccess) return fail_cuda(e, "grx_halo_z launch");
     return GRX_OK;
