@@ -179,6 +179,12 @@ int grx_valencia_rhs_zrange(const grx_grid* grid, const double* prim, const doub
                             void* cuda_stream);
 size_t grx_halo_z_bytes(const grx_grid* grid, int nghost);
 int grx_halo_z(const grx_grid* grid, double* prim, int nghost, int side, int unpack, double* buf, void* cuda_stream);
+/* grx_halo_z_pull: the peer-memory transport of the same exchange: one kernel that fills both sets of z ghost planes of `prim`
+ * by reading the neighbours' arrays directly -- below / above: DEVICE pointers to the prim arrays (same grid, same layout) of
+ * the slabs below and above, on this device or on a peer device whose memory is accessible from this one (NVLink peer
+ * access enabled by the caller).  No pack buffer and no staging copy.  The neighbours' x / y ghosts must be filled and their
+ * interior planes final when the kernel runs (order it with events).  A slab that is its own neighbour passes prim itself. */
+int grx_halo_z_pull(const grx_grid* grid, double* prim, int nghost, const double* below, const double* above, void* cuda_stream);
 int grx_fill_ghosts(const grx_grid* grid, double* prim, int nghost, int bc, int dirs, void* cuda_stream);
 int grx_rk_stage(const grx_grid* grid, int nghost, double a, const double* Ua, double b, const double* Ub, double h,
                  const double* L, double* Uout, double* acc, double wdt, const double* metric, double gamma, double* prim,

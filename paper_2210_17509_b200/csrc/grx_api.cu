@@ -447,6 +447,18 @@ int grx_tmunu_vertices(const grx_grid* grid, const double* prim, const double* m
     return GRX_OK;
 }
 
+int grx_halo_z_pull(const grx_grid* grid, double* prim, int nghost, const double* below, const double* above, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim || !below || !above) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (p.n[2] < p.g) return fail(GRX_ERR_INVALID_ARG, "a slab must have at least nghost planes");
+    if (p.nbox > 8191) return fail(GRX_ERR_INVALID_ARG, "grx_halo_z_pull takes at most 8191 boxes per call");
+    const cudaError_t e = grx::launch_halo_z_pull(p, prim, below, above, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return fail_cuda(e, "grx_halo_z_pull launch");
+    return GRX_OK;
+}
+
 size_t grx_ct_workspace_bytes(const grx_grid* grid, int nghost) {
     grx::RhsParams p;
     std::memset(&p, 0, sizeof(p));

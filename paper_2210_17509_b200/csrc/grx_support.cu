@@ -135,6 +135,21 @@ __global__ void __launch_bounds__(256) halo_z_kernel(const __grid_constant__ Rhs
     if (unpack) *a = *b; else *b = *a;
 }
 
+// NEXT-4, peer-memory transport: the z ghost planes are PULLED straight out of the neighbours' arrays -- `below` and `above`
+// are the prim arrays of the slabs below and above (same shape), on this device or on a peer whose memory is mapped
+// (NVLink peer access): no pack buffer, no staging copy, one kernel.  low ghost planes <- the g highest interior planes of
+// `below`, high ghost planes <- the g lowest interior planes of `above`.
+__global__ void __launch_bounds__(256) halo_z_pull_kernel(const __grid_constant__ RhsParams p, double* prim,
+                                                          const double* __restrict__ below, const double* __restrict__ above) {
+    const long long slab = (long long)p.g * p.stride[2];
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= slab) return;
+    const long long f = (long long)blockIdx.y * p.nc;   // box * 8 + field
+    const int side = blockIdx.z;
+    if (side == 0) prim[f + t] = below[f + (long long)p.n[2] * p.stride[2] + t];
+    else prim[f + (long long)(p.n[2] + p.g) * p.stride[2] + t] = above[f + (long long)p.g * p.stride[2] + t];
+}
+
 __global__ void selftest_math_kernel(const double* __restrict__ x, double* __restrict__ y, size_t n) {
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n) return;
@@ -205,6 +220,14 @@ cudaError_t launch_halo_z(const RhsParams& p, double* prim, double* buf, int sid
     if (slab == 0) return cudaSuccess;
     const dim3 grid((unsigned)((slab + 255) / 256), (unsigned)(p.nbox * 8));
     halo_z_kernel<<<grid, 256, 0, st>>>(p, prim, buf, side, unpack ? 1 : 0);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_halo_z_pull(const RhsParams& p, double* prim, const double* below, const double* above, cudaStream_t st) {
+    const long long slab = (long long)p.g * p.stride[2];
+    if (slab == 0) return cudaSuccess;
+    const dim3 grid((unsigned)((slab + 255) / 256), (unsigned)(p.nbox * 8), 2);
+    halo_z_pull_kernel<<<grid, 256, 0, st>>>(p, prim, below, above);
     return cudaGetLastError();
 }
 

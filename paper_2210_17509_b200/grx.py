@@ -19,7 +19,7 @@ VARIANT = {"auto": 0, "simple": 1, "ldg": 2, "tma": 3}
 EXPORTS = (
     "grx_valencia_rhs", "grx_valencia_rhs_host", "grx_host_workspace_bytes", "grx_prim2con", "grx_con2prim", "grx_rk_axpy",
     "grx_step_rk", "grx_step_workspace_bytes", "grx_step_rk_ct", "grx_step_ct_workspace_bytes", "grx_valencia_rhs_ct", "grx_ct_workspace_bytes",
-    "grx_valencia_rhs_vertex", "grx_tmunu_vertices", "grx_valencia_rhs_zrange", "grx_halo_z", "grx_halo_z_bytes", "grx_fill_ghosts", "grx_rk_stage", "grx_debug_set_fallback_counter",
+    "grx_valencia_rhs_vertex", "grx_tmunu_vertices", "grx_valencia_rhs_zrange", "grx_halo_z", "grx_halo_z_bytes", "grx_halo_z_pull", "grx_fill_ghosts", "grx_rk_stage", "grx_debug_set_fallback_counter",
     "grx_set_variant", "grx_selftest_math", "grx_dfma_peak_launch", "grx_fp64_issue_probe", "grx_last_error", "grx_version",
     "grx_weno_eps", "grx_v2max",
 )
@@ -62,6 +62,7 @@ def lib():
         L.grx_valencia_rhs_zrange.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, i, i, vp]
         L.grx_halo_z_bytes.argtypes = [gp, i]
         L.grx_halo_z.argtypes = [gp, vp, i, i, i, vp, vp]
+        L.grx_halo_z_pull.argtypes = [gp, vp, i, vp, vp, vp]
         L.grx_fill_ghosts.argtypes = [gp, vp, i, i, i, vp]
         L.grx_rk_stage.argtypes = [gp, i, dbl, vp, dbl, vp, dbl, vp, vp, vp, dbl, vp, dbl, vp, vp, vp]
         L.grx_valencia_rhs_vertex.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, vp]
@@ -264,6 +265,17 @@ def halo_z(prim, nghost, side, unpack, buf, stream=None):
     g = _grid(prim, nghost)
     _check(lib().grx_halo_z(C.byref(g), _dev(prim, 8), int(nghost), int(side), int(bool(unpack)),
                             C.c_void_p(buf.data_ptr()), _stream(stream)))
+
+
+def halo_z_pull(prim, nghost, below, above, stream=None):
+    """grx_halo_z_pull (NEXT-4, peer-memory transport): fills the z ghost planes of prim straight from the prim arrays of the
+    slabs below and above (same shape; this device or a peer with access enabled)."""
+    g = _grid(prim, nghost)
+    for t in (below, above):
+        if tuple(t.shape) != tuple(prim.shape):
+            raise GrxError("the neighbours' arrays must have the shape of prim")
+    _check(lib().grx_halo_z_pull(C.byref(g), _dev(prim, 8), int(nghost), C.c_void_p(below.data_ptr()),
+                                 C.c_void_p(above.data_ptr()), _stream(stream)))
 
 
 def fill_ghosts(prim, nghost, bc="periodic", dirs=7, stream=None):

@@ -50,8 +50,9 @@ class ZSlabExchange:
 
     @staticmethod
     def link_ring(exchanges):
-        """Emulates a ring of ranks inside ONE process (one GPU holding every slab; tests and single-GPU measurements):
-        exchanges[r] is rank r's object.  Protocol: start() on every slab, then finish() on every slab."""
+        """A ring of slabs inside ONE process (one GPU holding every slab, or one process driving several GPUs with peer
+        access): exchanges[r] is slab r's object.  On CUDA the transport is the peer-memory pull kernel grx_halo_z_pull
+        (no pack buffers, one kernel per slab).  Protocol: start() on every slab, then finish() on every slab."""
         for r, ex in enumerate(exchanges):
             ex._ring = (exchanges, r)
 
@@ -78,6 +79,15 @@ class ZSlabExchange:
         else:
             import contextlib
             ctx = contextlib.nullcontext()
+        self._pull = self._ring is not None and self.cuda and self._pack is None and self._unpack is None
+        if self._pull:
+            # peer-memory transport (grx_halo_z_pull): nothing to pack; the neighbours read this array directly once the
+            # compute stream has produced it
+            self._prim = prim
+            self._packed = torch.cuda.Event()
+            self._packed.record(self.stream)
+            self._reqs = []
+            return
         with ctx:
             self._do_pack(prim, 0, self.send[0])
             self._do_pack(prim, 1, self.send[1])
@@ -108,6 +118,15 @@ class ZSlabExchange:
         for r in self._reqs:
             r.wait()
         self._reqs = []
+        if self._ring is not None and getattr(self, "_pull", False):
+            from . import grx
+            ring, me = self._ring
+            below, above = ring[(me - 1) % len(ring)], ring[(me + 1) % len(ring)]
+            self.stream.wait_event(below._packed)
+            self.stream.wait_event(above._packed)
+            grx.halo_z_pull(prim, self.g, below._prim, above._prim, stream=self.stream)
+            (compute_stream or torch.cuda.current_stream()).wait_stream(self.stream)
+            return
         if self._ring is not None:
             ring, me = self._ring
             below, above = ring[(me - 1) % len(ring)], ring[(me + 1) % len(ring)]

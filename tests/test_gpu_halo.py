@@ -150,3 +150,24 @@ def test_halo_pack_unpack_roundtrip(grx):
         mask = torch.ones_like(q, dtype=torch.bool)
         mask[:, :, k_ghost:k_ghost + g] = False
         assert torch.equal(q[mask], prim[mask])
+
+
+def test_halo_pull_matches_pack_and_unpack(grx):
+    """The peer-memory transport (grx_halo_z_pull) fills the ghost planes with the bits of pack / copy / unpack, touches
+    nothing else, and a slab that is its own neighbour wraps around."""
+    import torch
+    g = 3
+    shape = (1, 8, 15, 9, 10)
+    slabs = [torch.randn(shape, dtype=torch.float64, device="cuda") for _ in range(3)]
+    nz = shape[2] - 2 * g
+    for me in range(3):
+        below, above = slabs[(me - 1) % 3], slabs[(me + 1) % 3]
+        got = slabs[me].clone()
+        grx.halo_z_pull(got, g, below, above)
+        exp = slabs[me].clone()
+        exp[:, :, :g] = below[:, :, nz:nz + g]
+        exp[:, :, nz + g:] = above[:, :, g:2 * g]
+        assert torch.equal(got, exp)
+    own = slabs[0].clone()
+    grx.halo_z_pull(own, g, own, own)
+    assert torch.equal(own[:, :, :g], slabs[0][:, :, nz:nz + g]) and torch.equal(own[:, :, nz + g:], slabs[0][:, :, g:2 * g])
