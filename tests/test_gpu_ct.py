@@ -77,6 +77,17 @@ def test_ct_parity_ragged_and_thin(grx, oracle, n):
             _check(prob, recon, got, plain, fb, oracle)
 
 
+def test_ct_two_and_four_ghosts(grx, oracle):
+    """nghost = 2 (the minimum for minmod / MC: the faces of the lines next to the block reach the outermost ghost cells) and
+    nghost = 4 (wider than needed)."""
+    for g, recons in ((2, ("minmod", "mc")), (4, ("weno5", "minmod"))):
+        prob = inputs.general_metric_box(n=(34, 11, 9), seed=27, g=g, nbox=2)
+        for variant in ("auto", "tma", "ldg"):
+            for recon in recons:
+                got, plain, fb = _run(grx, prob, recon, variant)
+                _check(prob, recon, got, plain, fb, oracle)
+
+
 def test_ct_update_is_divergence_free_on_the_gpu(grx):
     """The vertex-centred divergence of the GPU's d calB/dt vanishes to rounding on a multi-tile block."""
     prob = inputs.general_metric_box(n=(70, 30, 21), seed=17)
