@@ -470,6 +470,10 @@ def run_ours(args):
     recon = args.recon
     host = [torch.from_numpy(np.ascontiguousarray(a)) for a in (prob.prim, prob.metric, prob.K)]
     dev = tuple(t.cuda() for t in host)
+    if rank != 0:
+        # only rank 0 runs the oracle: the other ranks keep one (pinned) host copy of their inputs, not two
+        host = [t.pin_memory() for t in host]
+        prob.prim = prob.metric = prob.K = None
     cells = prob.cells
     g = prob.nghost
 
@@ -499,7 +503,7 @@ def run_ours(args):
 
     # ---- end to end through grx_valencia_rhs_host: pinned host buffers, H2D + kernel + D2H per step
     e2e_steps = max(1, min(args.steps, 5))
-    hp, hm, hk = (t.pin_memory() for t in host)
+    hp, hm, hk = (t if t.is_pinned() else t.pin_memory() for t in host)
     ho = torch.empty_like(hp).pin_memory()
     ws = torch.empty(grx.host_workspace_bytes(hp.shape, g) // 8, dtype=torch.float64, device="cuda")
     grx.valencia_rhs_host(hp, hm, hk, prob.dx, g, recon, prob.gamma, ho, ws, stream=stream)
