@@ -91,9 +91,11 @@ int grx_valencia_rhs(const grx_grid* grid, const double* prim, const double* met
  * along z are processed as a pipeline of 32-plane slabs: the upload of the next slab, the kernel of the current
  * one and the download of the previous one overlap on three streams (two internal ones per host thread and
  * device, created on first use and kept, ordered after / before `cuda_stream` by events); the results are bitwise
- * those of the device entry point.  Only the INTERIOR planes of `out_host` are written in that case (all of it, ghosts holding whatever
- * the workspace held, for blocks of <= 32 planes or while a debug fallback counter is set).  The host arrays
- * have the layout above and should be page-locked for the copies to be asynchronous.
+ * those of the device entry point on the interior cells.  Ghost cells of `out_host` (unlike those of the device entry
+ * point's `out`) are NOT preserved: in the pipelined case the planes k = nghost .. nz + nghost - 1 are copied back whole, so
+ * their x and y ghost cells receive whatever the workspace held, and the z ghost planes are left alone; for blocks of <= 32
+ * planes, or while a debug fallback counter is set, the whole array is copied back.  The host arrays have the layout above
+ * and should be page-locked for the copies to be asynchronous.
  *   workspace        DEVICE pointer, at least grx_host_workspace_bytes(grid, nghost) bytes, owned by the caller.
  * Results are valid in out_host after `cuda_stream` is synchronised. */
 size_t grx_host_workspace_bytes(const grx_grid* grid, int nghost);
