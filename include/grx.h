@@ -4,13 +4,13 @@
  * line numbers): "reconstruct -> Riemann -> flux divergence + source" (steps 2-4, l.127-132) of the
  * Valencia formulation, Eqs. (6)-(13) (l.86-114), with TVD/WENO5 reconstruction (l.130, l.134), the
  * HLLE solver (l.131, l.136) and an ideal-gas Gamma-law EOS (l.138).  Readings of everything the paper
- * leaves open (R1..R29) are listed in DESIGN.md.
+ * leaves open (R1..R32) are listed in DESIGN.md.
  *
  * Conventions shared by every entry point
  * ---------------------------------------
  *  - Every array pointer is a DEVICE pointer to FP64 unless it says HOST.  The caller owns all memory;
  *    the library never allocates, frees or keeps user memory.  grx_valencia_rhs and grx_prim2con need no
- *    workspace; the host entry point grx_valencia_rhs_host takes one from the caller.
+ *    workspace; the host, time-stepping and constrained-transport entry points take one from the caller.
  *  - State: none between calls, except three debug/plumbing items that are stated where they are declared: the
  *    process-wide kernel selector (grx_set_variant, default AUTO), the per-thread fallback counter pointer
  *    (grx_debug_set_fallback_counter) and two per-thread CUDA streams that grx_valencia_rhs_host creates on
@@ -25,7 +25,8 @@
  *        metric[10]: alp, beta^x, beta^y, beta^z, g_xx, g_xy, g_xz, g_yy, g_yz, g_zz   (ADM, l.56)
  *        K     [6] : K_xx, K_xy, K_xz, K_yy, K_yz, K_zz   (d_t g_ij = -2 alp K_ij + Lie_beta g_ij, R12)
  *        cons/out[8]: D, S_x, S_y, S_z, tau, calB^x, calB^y, calB^z  (densitised, Eqs. 6-9 l.88-94)
- *    Metric and K are co-located with the fluid at cell centres (R6).
+ *    Metric and K are co-located with the fluid at cell centres (R6), except in the two vertex-centred entry points
+ *    (grx_valencia_rhs_vertex, grx_tmunu_vertices: R31 / R32), which say so.
  *  - Calls are asynchronous on `cuda_stream` (a cudaStream_t; NULL = the legacy default stream); results
  *    are valid after that stream is synchronised.
  *  - Errors: every entry point returns a code, never aborts or throws.  Arguments are validated on the
