@@ -86,9 +86,11 @@ GRX_HD void recon_cell(double a, double b, double c, double d, double e, double&
         // 4*beta_k + 4 eps = 13/3 t_k^2 + u_k^2 + 4 eps  (the common factor 4 cancels in the weights; the epsilon rides
         // on the inner FMA)
         const double k133 = 13.0 / 3.0, eps4 = 4.0 * WENO_EPS;
-        double e0 = fma(k133 * t0, t0, fma(u0, u0, eps4));
-        double e1 = fma(k133 * t1, t1, fma(u1, u1, eps4));
-        double e2 = fma(k133 * t2, t2, fma(u2, u2, eps4));
+        // t^2 first, then the constant as an FMA operand: a DFMA with a constant operand occupies the pipe 2 cycles, one with
+        // three registers 3 (profiles/r2_issue_model.md)
+        double e0 = fma(t0 * t0, k133, fma(u0, u0, eps4));
+        double e1 = fma(t1 * t1, k133, fma(u1, u1, eps4));
+        double e2 = fma(t2 * t2, k133, fma(u2, u2, eps4));
         e0 *= e0; e1 *= e1; e2 *= e2;
         // a_k = d_k / e_k  ->  multiply all three by e0 e1 e2 (common denominator, R26)
         const double e01 = e0 * e1, e02 = e0 * e2, e12 = e1 * e2;
