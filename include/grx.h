@@ -14,7 +14,8 @@
  *  - State: none between calls, except three debug/plumbing items that are stated where they are declared: the
  *    process-wide kernel selector (grx_set_variant, default AUTO), the per-thread fallback counter pointer
  *    (grx_debug_set_fallback_counter) and two per-thread CUDA streams that grx_valencia_rhs_host creates on
- *    first use.  No environment variable is read.  Entry points may be called from several host threads and on
+ *    first use; plus the fixed device array of grx_valencia_rhs_ct_static and its per-device address.  No environment
+ *    variable is read.  Entry points may be called from several host threads and on
  *    several devices (the current device of the calling thread is used).
  *  - Layout: structure of arrays, x fastest, ghost zones included, boxes contiguous:
  *        a[box][field][k][j][i],   i in [0,Nx), j in [0,Ny), k in [0,Nz),   N* = n* + 2*nghost,
@@ -161,6 +162,42 @@ size_t grx_ct_workspace_bytes(const grx_grid* grid, int nghost);
 int grx_valencia_rhs_ct(const grx_grid* grid, const double* prim, const double* metric, const double* K,
                         const double dx[3], int nghost, int recon, double gamma, double* out, void* workspace,
                         size_t workspace_bytes, void* cuda_stream);
+
+/* grx_valencia_rhs_ct for callers that have no device memory to give and may not ask the driver for any.
+ *
+ * Who that is: in the setting this method comes from, one component of the host code owns device memory -- the paper's
+ * driver "handles all data movement and memory allocations" (l.154) and calls user functions on blocks of data -- and such
+ * drivers commonly reserve most of HBM for their own arena at start-up, so cudaMalloc may have nothing left to return.  A
+ * routine called from inside that time loop, through an interface that passes field pointers only, or from a region where
+ * the device-wide synchronisation implied by cudaMalloc / cudaFree would stall every other stream, cannot size and
+ * allocate the six face-flux arrays that grx_valencia_rhs_ct wants as `workspace`.  This entry point keeps those arrays inside the library instead:
+ * in ONE fixed array of GRX_CT_STATIC_MAX_BYTES (16 MiB) of device memory that is part of the loaded library image.  Every
+ * GPU on which the process uses the library holds these 16 MiB from the moment the library's code is loaded there until
+ * the process exits, whether or not this entry point is ever called.
+ *
+ *   - It calls no cudaMalloc, cudaFree or any other allocating routine, on any call.  prim, metric, K and out are the
+ *     caller's, exactly as for grx_valencia_rhs_ct; results are the same bits as grx_valencia_rhs_ct gives.
+ *   - Limit: 6 * (nx + 2 nghost)(ny + 2 nghost)(nz + 2 nghost) * nbox * 8 bytes <= GRX_CT_STATIC_MAX_BYTES, i.e. at most
+ *     349 525 cells (ghosts included) summed over the boxes of the call -- one 64^3 block with 3 ghost cells (70^3 = 343 000)
+ *     fits, so do 4 x 38^3.  A larger call returns GRX_ERR_INVALID_ARG ("... exceeds the static scratch ...") and launches
+ *     nothing: split it into several calls, or use grx_valencia_rhs_ct with your own workspace.
+ *   - First call on each device: the library looks up the device address of the array once per device (with the calling
+ *     thread's current device) and keeps it.  That look-up makes the CUDA runtime load the library's device code on that
+ *     device if it has not yet done so.  Make this first call during start-up, before any stream capture begins.
+ *   - All calls on one device share the one array, from every thread and every stream.  Two calls whose kernels can be on
+ *     the GPU at the same time (different streams without an ordering between them, or two host threads) overwrite each
+ *     other's face fluxes and both results are garbage: order them on one stream or with events.  Calls on different
+ *     devices do not interact.
+ *   - The array keeps what the previous call left in it.  Nothing in it has to start at zero: each call writes every
+ *     face flux it later reads (faces of the interior grid lines by the right-hand-side kernel, the one layer next to the
+ *     block by the face kernel) before the curl kernel runs, so stale contents are never read.  The face fluxes are not
+ *     returned; a caller that wants them uses grx_valencia_rhs_ct.
+ * grx_ct_static_max_bytes() returns GRX_CT_STATIC_MAX_BYTES (for bindings that cannot see the macro).
+ * Other arguments, return codes and asynchrony as for grx_valencia_rhs_ct. */
+#define GRX_CT_STATIC_MAX_BYTES ((size_t)16 << 20)
+size_t grx_ct_static_max_bytes(void);
+int grx_valencia_rhs_ct_static(const grx_grid* grid, const double* prim, const double* metric, const double* K,
+                               const double dx[3], int nghost, int recon, double gamma, double* out, void* cuda_stream);
 
 /* NEXT-4 (PAPER.md l.222-230 ghost-zone fill between blocks, l.371 "start the computations of those
  * cells ... which do not need ghost cells while ghost cells ... are getting filled, and then compute the remaining cells

@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "../../include/grx.h"
@@ -130,6 +131,37 @@ cudaError_t launch_rhs_ct(grx::RhsParams p, int recon, cudaStream_t st, bool* un
     if (e == cudaSuccess) e = grx::launch_face_bflux(p, recon, !fused_faces, st);
     if (e == cudaSuccess) e = grx::launch_flux_ct(p, st);
     return e;
+}
+
+// ---- grx_valencia_rhs_ct_static: the face-flux scratch of constrained transport as part of the library image ----------
+// For callers that cannot allocate device memory (include/grx.h says who and why).  The array below lives in the device
+// image of this translation unit: every device that loads the library carries its 16 MiB until the process ends.
+// In host code the NAME of a __device__ array is only a handle for the runtime -- it is not an address the GPU can use; a
+// kernel handed `g_ct_static_scratch` from the host would fault or scribble over unrelated memory.  The device address
+// comes from cudaGetSymbolAddress, asked once per device with that device current, and is what the kernels receive.
+constexpr size_t CT_STATIC_DOUBLES = GRX_CT_STATIC_MAX_BYTES / sizeof(double);
+static __device__ __align__(256) double g_ct_static_scratch[CT_STATIC_DOUBLES];
+
+constexpr int CT_STATIC_MAX_DEVICES = 64;
+std::mutex g_ct_static_mutex;
+double* g_ct_static_addr[CT_STATIC_MAX_DEVICES] = {};   // device address of the array on device i, nullptr = not asked yet
+
+// Device address of the scratch array on the calling thread's current device (looked up on the first call per device).
+cudaError_t ct_static_scratch(double** addr) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= CT_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_ct_static_mutex);
+    if (!g_ct_static_addr[dev]) {
+        void* a = nullptr;
+        e = cudaGetSymbolAddress(&a, g_ct_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (!a) return cudaErrorInvalidSymbol;
+        g_ct_static_addr[dev] = static_cast<double*>(a);
+    }
+    *addr = g_ct_static_addr[dev];
+    return cudaSuccess;
 }
 
 }  // namespace
@@ -494,6 +526,50 @@ int grx_valencia_rhs_ct(const grx_grid* grid, const double* prim, const double* 
     const cudaError_t e = launch_rhs_ct(p, recon, st, &unsupported);
     if (unsupported) return fail(GRX_ERR_UNSUPPORTED, "GRX_VARIANT_TMA needs even nx + 2 nghost and 16-byte aligned arrays");
     if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_ct launch");
+    return GRX_OK;
+}
+
+size_t grx_ct_static_max_bytes(void) { return GRX_CT_STATIC_MAX_BYTES; }
+
+// Same checks and the same launch sequence as grx_valencia_rhs_ct; the six face-flux arrays go to the library's own fixed
+// device array instead of a caller's workspace.  No allocation on any call.  The array is shared by every call on the
+// device: calls that overlap on the GPU race (include/grx.h).  Nothing is cleared: launch_rhs_ct writes every face flux
+// the curl kernel reads before that kernel runs, whatever an earlier call left behind.
+int grx_valencia_rhs_ct_static(const grx_grid* grid, const double* prim, const double* metric, const double* K,
+                               const double dx[3], int nghost, int recon, double gamma, double* out, void* cuda_stream) {
+    grx::RhsParams p;
+    std::memset(&p, 0, sizeof(p));
+    if (const char* why = make_geom(grid, nghost, p)) return fail(GRX_ERR_INVALID_ARG, why);
+    if (!prim || !metric || !K || !dx || !out) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
+    if (recon != GRX_RECON_MINMOD && recon != GRX_RECON_MC && recon != GRX_RECON_WENO5)
+        return fail(GRX_ERR_INVALID_ARG, "unknown recon");
+    if (nghost < (recon == GRX_RECON_WENO5 ? 3 : 2))
+        return fail(GRX_ERR_INVALID_ARG, "nghost too small: WENO5 needs 3, minmod/MC need 2 (R29)");
+    if (!(gamma > 1.0)) return fail(GRX_ERR_INVALID_ARG, "gamma must be > 1");
+    for (int a = 0; a < 3; ++a) {
+        if (!(dx[a] > 0.0) || !(1.0 / dx[a] > 0.0)) return fail(GRX_ERR_INVALID_ARG, "dx must be > 0 and finite");
+        p.idx[a] = 1.0 / dx[a];
+    }
+    if (out == prim || out == metric || out == K) return fail(GRX_ERR_INVALID_ARG, "out must not alias an input");
+    const unsigned long long need = 6ULL * (unsigned long long)p.nc * (unsigned long long)p.nbox;   // <= 6 * 2^31 * 2^16
+    if (need > CT_STATIC_DOUBLES) {
+        std::snprintf(t_err, sizeof(t_err),
+                      "the call needs %llu bytes of face fluxes, which exceeds the static scratch of %llu bytes "
+                      "(GRX_CT_STATIC_MAX_BYTES): split the call or use grx_valencia_rhs_ct with a workspace",
+                      need * 8ULL, (unsigned long long)GRX_CT_STATIC_MAX_BYTES);
+        return GRX_ERR_INVALID_ARG;
+    }
+    double* scratch = nullptr;
+    cudaError_t e = ct_static_scratch(&scratch);
+    if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_ct_static: address of the static scratch");
+    p.prim = prim; p.met = metric; p.K = K; p.out = out;
+    p.gamma = gamma;
+    p.nfallback = t_fallback_counter;
+    p.fb = scratch;
+    bool unsupported = false;
+    e = launch_rhs_ct(p, recon, static_cast<cudaStream_t>(cuda_stream), &unsupported);
+    if (unsupported) return fail(GRX_ERR_UNSUPPORTED, "GRX_VARIANT_TMA needs even nx + 2 nghost and 16-byte aligned arrays");
+    if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_ct_static launch");
     return GRX_OK;
 }
 

@@ -19,6 +19,7 @@ VARIANT = {"auto": 0, "simple": 1, "ldg": 2, "tma": 3}
 EXPORTS = (
     "grx_valencia_rhs", "grx_valencia_rhs_host", "grx_host_workspace_bytes", "grx_prim2con", "grx_con2prim", "grx_rk_axpy",
     "grx_step_rk", "grx_step_workspace_bytes", "grx_step_rk_ct", "grx_step_ct_workspace_bytes", "grx_valencia_rhs_ct", "grx_ct_workspace_bytes",
+    "grx_valencia_rhs_ct_static", "grx_ct_static_max_bytes",
     "grx_valencia_rhs_vertex", "grx_tmunu_vertices", "grx_valencia_rhs_zrange", "grx_halo_z", "grx_halo_z_bytes", "grx_halo_z_pull", "grx_fill_ghosts", "grx_rk_stage", "grx_debug_set_fallback_counter",
     "grx_set_variant", "grx_selftest_math", "grx_dfma_peak_launch", "grx_fp64_issue_probe", "grx_last_error", "grx_version",
     "grx_weno_eps", "grx_v2max",
@@ -59,6 +60,8 @@ def lib():
         L.grx_step_ct_workspace_bytes.argtypes = [gp, i, i]
         L.grx_ct_workspace_bytes.argtypes = [gp, i]
         L.grx_valencia_rhs_ct.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, vp, sz, vp]
+        L.grx_valencia_rhs_ct_static.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, vp]
+        L.grx_ct_static_max_bytes.argtypes = []
         L.grx_valencia_rhs_zrange.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, i, i, vp]
         L.grx_halo_z_bytes.argtypes = [gp, i]
         L.grx_halo_z.argtypes = [gp, vp, i, i, i, vp, vp]
@@ -78,6 +81,7 @@ def lib():
         L.grx_step_workspace_bytes.restype = sz
         L.grx_step_ct_workspace_bytes.restype = sz
         L.grx_ct_workspace_bytes.restype = sz
+        L.grx_ct_static_max_bytes.restype = sz
         L.grx_halo_z_bytes.restype = sz
         L.grx_last_error.restype = C.c_char_p
         L.grx_weno_eps.restype = dbl
@@ -153,6 +157,30 @@ def valencia_rhs_ct(prim, metric, K, dx, nghost, recon, gamma, out=None, workspa
                                      float(gamma), _dev(out, 8), C.c_void_p(workspace.data_ptr()),
                                      workspace.numel() * workspace.element_size(), _stream(stream)))
     return out, workspace
+
+
+def ct_static_max_bytes():
+    """GRX_CT_STATIC_MAX_BYTES: the size of the library's built-in face-flux array (16 MiB)."""
+    return lib().grx_ct_static_max_bytes()
+
+
+def valencia_rhs_ct_static(prim, metric, K, dx, nghost, recon, gamma, out, stream=None):
+    """grx_valencia_rhs_ct_static: valencia_rhs_ct for callers that cannot allocate device memory -- a code whose driver
+    owns all of HBM, a callback that is handed field pointers only, a region where cudaMalloc's device-wide
+    synchronisation is not acceptable.  The six face-flux arrays live in a fixed 16 MiB device array inside libgrx.so, so
+    neither this wrapper nor the library allocates anything: `out` is required (same shape as prim), and the call is
+    refused with GrxError when 6 * cells (ghosts included, all boxes) * 8 bytes exceeds ct_static_max_bytes().
+    Make the first call on a device during start-up (it looks up the array's device address, once per device).  All calls
+    on a device share the array: order them on one stream, overlapping calls corrupt each other.  Returns `out`."""
+    g = _grid(prim, nghost)
+    if metric.shape[0] != prim.shape[0] or K.shape[0] != prim.shape[0] or metric.shape[2:] != prim.shape[2:] \
+            or K.shape[2:] != prim.shape[2:] or out.shape != prim.shape:
+        raise GrxError("prim, metric, K, out must share nbox and the spatial shape")
+    r = RECON[recon] if isinstance(recon, str) else int(recon)
+    dxa = (C.c_double * 3)(*[float(v) for v in dx])
+    _check(lib().grx_valencia_rhs_ct_static(C.byref(g), _dev(prim, 8), _dev(metric, 10), _dev(K, 6), dxa, int(nghost), r,
+                                            float(gamma), _dev(out, 8), _stream(stream)))
+    return out
 
 
 def host_workspace_bytes(shape, nghost):
