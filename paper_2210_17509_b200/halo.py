@@ -46,6 +46,8 @@ class ZSlabExchange:
         self._reqs = []
         self._ring = None          # in-process ring (link_ring): the slabs of several "ranks" live in this process
         self._packed = None
+        self._cs = None            # compute stream of the exchange in flight (pull transport: the neighbours order on it)
+        self._prim = None
         self.bytes_per_exchange = 2 * self.send[0].numel() * self.send[0].element_size()
 
     @staticmethod
@@ -74,6 +76,7 @@ class ZSlabExchange:
         import torch
         if self.cuda:
             cs = compute_stream or torch.cuda.current_stream()
+            self._cs = cs
             self.stream.wait_stream(cs)          # prim is final on the compute stream
             ctx = torch.cuda.stream(self.stream)
         else:
@@ -115,8 +118,17 @@ class ZSlabExchange:
     def finish(self, prim, compute_stream=None):
         """Completes the exchange: the z ghost planes of `prim` are filled for later work on the compute stream."""
         import torch
-        for r in self._reqs:
-            r.wait()
+        if self._reqs:
+            # Work.wait() of the NCCL backend does not block the host: it makes the CURRENT stream wait for the transfer.
+            # The unpack kernels run on self.stream, so that is the stream that has to be current here (gloo blocks the
+            # host instead, where any stream will do).
+            if self.cuda:
+                with torch.cuda.stream(self.stream):
+                    for r in self._reqs:
+                        r.wait()
+            else:
+                for r in self._reqs:
+                    r.wait()
         self._reqs = []
         if self._ring is not None and getattr(self, "_pull", False):
             from . import grx
@@ -125,6 +137,15 @@ class ZSlabExchange:
             self.stream.wait_event(below._packed)
             self.stream.wait_event(above._packed)
             grx.halo_z_pull(prim, self.g, below._prim, above._prim, stream=self.stream)
+            # the pull read the neighbours' arrays: whatever their compute streams enqueue from now on (the next stage
+            # writes prim) is ordered after it.  The protocol (every start() before any finish(), the next writes after
+            # every finish()) makes "from now on" early enough.
+            pulled = torch.cuda.Event()
+            pulled.record(self.stream)
+            for nb in (below, above):
+                if nb is not self and nb._cs is not None:
+                    nb._cs.wait_event(pulled)
+            # self._prim stays set: the neighbours' finish() calls, which come later, read it
             (compute_stream or torch.cuda.current_stream()).wait_stream(self.stream)
             return
         if self._ring is not None:
@@ -175,6 +196,13 @@ def step_rk2_zslabs(exch, cons, prim, metric, K, dx, nghost, recon, gamma, dt, n
     fill (grx_fill_ghosts, dirs = 3).  `prim` must come with filled x / y ghosts; its z ghosts are exchanged here.
     work: two arrays shaped like cons (U0 and L)."""
     from . import grx
+    if stream is not None and cons.is_cuda:
+        import torch
+        if stream != torch.cuda.current_stream(cons.device):
+            # U0.copy_ below is a torch operation and goes to torch's current stream: make `stream` that stream
+            with torch.cuda.stream(stream):
+                return step_rk2_zslabs(exch, cons, prim, metric, K, dx, nghost, recon, gamma, dt, nsteps, work, overlap,
+                                       nfail, stream)
     U0, L = work
     for _ in range(nsteps):
         U0.copy_(cons)
