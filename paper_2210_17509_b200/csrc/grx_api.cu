@@ -61,8 +61,7 @@ int choose_kernel(const grx::RhsParams& p, int recon) {
     // set-up fill the SMs less well than the LDG kernel's 11-row tiles (constants fitted on the config-5 sweep,
     // profiles/r2_sweep.md: the selector picks the faster kernel at every point).
     int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess &&
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) {
+    if (grx::current_device_sms(&dev, &sms) == cudaSuccess) {
         const double gain = (recon == GRX_RECON_WENO5) ? 1.12 : 1.22;
         if (gain * grx::tma_tile_efficiency(p, sms) < grx::fused_tile_efficiency(p, sms)) return 1;
     }
@@ -80,6 +79,14 @@ cudaError_t launch_variant(const grx::RhsParams& p, int recon, cudaStream_t st, 
             if (unsupported) *unsupported = true;
             return cudaErrorNotSupported;
     }
+}
+
+// Launches kernel `kernel` (a choose_kernel result >= 0 taken on the WHOLE block) on a block or on a z sub-block of it.
+// nz_whole: interior planes of the whole block -- the LDG kernel picks its row tile from it, so that every plane of a
+// sub-block carries the bits of the whole-block call (the two kernels, and the tiles of one, round differently).
+cudaError_t launch_chosen(int kernel, const grx::RhsParams& p, int recon, cudaStream_t st, int nz_whole) {
+    return kernel == 0 ? grx::launch_rhs_simple(p, recon, st)
+         : kernel == 1 ? grx::launch_rhs_fused(p, recon, st, nz_whole) : grx::launch_rhs_tma(p, recon, 7, st);
 }
 
 // The two internal streams of grx_valencia_rhs_host: one pair per host thread and device, created on first use.
@@ -248,9 +255,13 @@ int grx_valencia_rhs_host(const grx_grid* grid, const double* prim_host, const d
         if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_host D2H");
         return GRX_OK;
     }
+    // One kernel choice for all slabs, taken on the whole block as the device entry point takes it: the selector looks at
+    // the geometry (a 32-plane slab fills the machine differently from the block), and results must not depend on it.
+    const int kernel = choose_kernel(p, recon);
+    if (kernel < 0) return fail(GRX_ERR_UNSUPPORTED, "GRX_VARIANT_TMA needs even nx + 2 nghost and 16-byte aligned arrays");
     cudaStream_t s_up = nullptr, s_dn = nullptr;
     cudaEvent_t ev_start = nullptr, ev_dn = nullptr;
-    // a tail shorter than 8 planes joins the last full slab, so that every slab takes the same tile as the whole block
+    // a tail shorter than 8 planes joins the last full slab (no slab thinner than the stencil work it amortises)
     const int nchunk = (Nz + CH - 1) / CH, nslab = (nz % CH != 0 && nz % CH < 8) ? nz / CH : (nz + CH - 1) / CH;
     std::vector<cudaEvent_t> ev_up(nchunk, nullptr), ev_done(nslab, nullptr);
     cudaError_t e = host_streams(&s_up, &s_dn);
@@ -289,7 +300,7 @@ int grx_valencia_rhs_host(const grx_grid* grid, const double* prim_host, const d
         ps.prim = d_prim + off; ps.met = d_met + off; ps.K = d_K + off; ps.out = d_out + off;
         ps.n[2] = k1 - k0;
         ps.N[2] = (k1 - k0) + 2 * g;
-        e = launch_variant(ps, recon, st);
+        e = launch_chosen(kernel, ps, recon, st, nz);
         if (e == cudaSuccess) e = cudaEventRecord(ev_done[i], st);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(s_dn, ev_done[i], 0);
         const size_t ooff = (size_t)(k0 + g) * plane, obytes = (size_t)(k1 - k0) * plane * sizeof(double);
@@ -382,8 +393,7 @@ int grx_valencia_rhs_zrange(const grx_grid* grid, const double* prim, const doub
     p.n[2] = k_end - k_begin;
     p.N[2] = p.n[2] + 2 * p.g;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    cudaError_t e = kernel == 0 ? grx::launch_rhs_simple(p, recon, st)
-                  : kernel == 1 ? grx::launch_rhs_fused(p, recon, st, nz_whole) : grx::launch_rhs_tma(p, recon, 7, st);
+    const cudaError_t e = launch_chosen(kernel, p, recon, st, nz_whole);
     if (e != cudaSuccess) return fail_cuda(e, "grx_valencia_rhs_zrange launch");
     return GRX_OK;
 }

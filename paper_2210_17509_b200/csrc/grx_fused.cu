@@ -304,17 +304,16 @@ TileGeom make_tiles(const RhsParams& p, int ty, int slots, double* eff_out = nul
     return tg;
 }
 
-// No cached state: the SM count and the shared-memory opt-in are per device and are queried / set on every launch
-// (both are cheap), so the library works with several devices and from several host threads.
+// The SM count and the shared-memory opt-in are per device: both are asked / set once per device and remembered
+// (grx_launch.h; lock-free, so the library still works with several devices and from several host threads).
 template <int RECON, int TY, int MINB, bool VERTEX>
 cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
     int dev = 0, sms = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaError_t e = current_device_sms(&dev, &sms);
     if (e != cudaSuccess) return e;
     const size_t smem = 2 * sizeof(Exch<TY>) + PARK_SLOTS * (TY + 1) * 32 * sizeof(double);
-    e = cudaFuncSetAttribute(rhs_fused_kernel<RECON, TY, MINB, VERTEX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static std::atomic<unsigned long long> smem_set{0};   // per instantiation: devices on which the attribute is set
+    e = set_max_dynamic_smem_once(rhs_fused_kernel<RECON, TY, MINB, VERTEX>, dev, smem, smem_set);
     if (e != cudaSuccess) return e;
     const TileGeom tg = make_tiles(p, TY, sms * MINB);
     const dim3 grid((unsigned)(tg.ntx * tg.nty * tg.nzc), p.nbox);

@@ -1,11 +1,45 @@
 // grx_launch.h -- internal: host-side launchers implemented by the kernel translation units.
 #pragma once
 
+#include <atomic>
+
 #include <cuda_runtime.h>
 
 #include "grx_common.cuh"
 
 namespace grx {
+
+// Current device of the calling thread and its SM count.  The count is asked from the runtime once per device and kept
+// (lock-free; a launch needs it two or three times, and the query is a visible share of a small block's launch latency).
+constexpr int MAX_CACHED_DEVICES = 64;
+inline cudaError_t current_device_sms(int* dev_out, int* sms_out) {
+    static std::atomic<int> cache[MAX_CACHED_DEVICES];   // zero-initialised: 0 = not asked yet
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool cached = dev >= 0 && dev < MAX_CACHED_DEVICES;
+    int sms = cached ? cache[dev].load(std::memory_order_relaxed) : 0;
+    if (sms <= 0) {
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        if (sms <= 0) return cudaErrorInvalidDevice;
+        if (cached) cache[dev].store(sms, std::memory_order_relaxed);
+    }
+    *dev_out = dev;
+    *sms_out = sms;
+    return cudaSuccess;
+}
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) of one kernel instantiation, once per device: `done` is that
+// instantiation's bit mask over devices (a function-local static of its launcher).
+template <typename Kernel>
+inline cudaError_t set_max_dynamic_smem_once(Kernel kernel, int dev, size_t smem, std::atomic<unsigned long long>& done) {
+    const bool tracked = dev >= 0 && dev < MAX_CACHED_DEVICES;
+    if (tracked && (done.load(std::memory_order_acquire) >> dev & 1ULL)) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess && tracked) done.fetch_or(1ULL << dev, std::memory_order_release);
+    return e;
+}
 
 // grx_simple.cu: one thread per cell, every thread evaluates its own six faces (cross-check variant)
 cudaError_t launch_rhs_simple(const RhsParams& p, int recon, cudaStream_t st);

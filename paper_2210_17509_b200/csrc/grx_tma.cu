@@ -564,18 +564,15 @@ template <int RECON, int TY, bool CT>
 cudaError_t launch_one(const RhsParams& p, cudaStream_t st) {
     using L = Lay<RECON, TY>;
     int dev = 0, sms = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaError_t e = current_device_sms(&dev, &sms);
     if (e != cudaSuccess) return e;
     CUtensorMap tmP, tmM, tmK;
     if (!make_map(&tmP, p.prim, p, 8, L::PW, L::PR) || !make_map(&tmM, p.met, p, 10, L::MW, L::MR) ||
         !make_map(&tmK, p.K, p, 6, TX + 2, TY))
         return cudaErrorNotSupported;
     const size_t smem = (size_t)L::total * sizeof(double);
-    // per device and cheap: set on every launch (no cached state, safe with several devices and host threads)
-    // per device and cheap: set on every launch (no cached state, safe with several devices and host threads)
-    e = cudaFuncSetAttribute(rhs_tma_kernel<RECON, TY, CT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static std::atomic<unsigned long long> smem_set{0};   // per instantiation: devices on which the attribute is set
+    e = set_max_dynamic_smem_once(rhs_tma_kernel<RECON, TY, CT>, dev, smem, smem_set);
     if (e != cudaSuccess) return e;
     const TmaGeom tg = make_tiles(p, TY, sms);
     const dim3 grid((unsigned)(tg.ntx * tg.nty * tg.nzc), p.nbox);

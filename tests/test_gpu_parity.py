@@ -558,6 +558,25 @@ def test_host_entry_point_pipelined(grx, oracle, n, nbox):
         assert np.all(got[:, :, :g] == -7.25e300) and np.all(got[:, :, -g:] == -7.25e300)
 
 
+@pytest.mark.parametrize("n,nbox", [((64, 64, 72), 1), ((32, 32, 100), 1), ((16, 4, 100), 3), ((128, 12, 40), 1),
+                                    ((96, 96, 33), 1), ((40, 40, 66), 2), ((33, 20, 41), 1), ((64, 64, 64), 16)])
+def test_host_entry_point_has_the_bits_of_the_device_entry_point(grx, n, nbox):
+    """The slab pipeline chooses its kernel (and the LDG kernel its row tile) once, on the whole block, as the device entry
+    point does: a 32-plane slab on its own would fill the machine differently and could be handed to the other kernel,
+    whose rounding differs.  Shapes around the selector's switch-over, small nx / ny with nz > 32, odd Nx, a sweep point."""
+    import torch
+    prob = inputs.sweep_boxes(n[0], nbox) if n[0] == n[1] == n[2] else inputs.general_metric_box(n=n, seed=5, nbox=nbox)
+    hp, hm, hk = (torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (prob.prim, prob.metric, prob.K))
+    ws = torch.empty(grx.host_workspace_bytes(hp.shape, prob.nghost) // 8, dtype=torch.float64, device="cuda")
+    ii = prob.interior
+    for recon in ("weno5", "minmod"):
+        ho = torch.zeros(hp.shape, dtype=torch.float64).pin_memory()
+        grx.valencia_rhs_host(hp, hm, hk, prob.dx, prob.nghost, recon, prob.gamma, ho, ws)
+        torch.cuda.synchronize()
+        dev = gpu_rhs(grx, prob, recon)
+        assert np.array_equal(ho.numpy()[ii], dev[ii]), (n, nbox, recon)
+
+
 def test_invalid_arguments_rejected(grx):
     import torch
     prob = inputs.general_metric_box(n=(8, 8, 8), seed=1)
