@@ -462,7 +462,8 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
                     face_geom_smem<MF, 1>(mx, m);
                     const long long cxr = cp + sy * xrow + xcol + 1;
                     face_flux<0>(m, PL, PR, prim + cxr - 1, prim + cxr, nc, gamma, Fh, count_x ? nfb : dup);
-                    if (CT) { fb[cxr] = Fh[6]; fb[nc + cxr] = Fh[7]; }
+                    // one writer per face: the face between two tiles is also the first face of the next tile's rows
+                    if (CT && count_x) { fb[cxr] = Fh[6]; fb[nc + cxr] = Fh[7]; }
 #pragma unroll
                     for (int q = 0; q < 8; ++q) fxo[q * TY] = Fh[q];
                 }
@@ -486,7 +487,9 @@ rhs_tma_kernel(const __grid_constant__ RhsParams p, const TmaGeom tg, const __gr
                 face_geom_smem<MF, MW>(myt, m);
                 const long long cyt = cp + lane + sy * tye;
                 face_flux<1>(m, PL, yt_qm, prim + cyt - sy, prim + cyt, nc, gamma, Fh, count_y ? nfb : dup);
-                if (CT) { fb[2 * nc + cyt] = Fh[5]; fb[3 * nc + cyt] = Fh[7]; }
+                // one writer per face: the face between two row tiles is written by row 0 of the tile above, whose
+                // inlined face_flux rounds differently from this one (two writers made the stored bits a race)
+                if (CT && count_y) { fb[2 * nc + cyt] = Fh[5]; fb[3 * nc + cyt] = Fh[7]; }
 #pragma unroll
                 for (int q = 0; q < 8; ++q) QF[q * EF + tye * 32 + lane] = Fh[q];
             }
