@@ -176,3 +176,43 @@ def test_balsara_2_to_5_start_admissibly(oracle, test, cfl):
     t_over_dx = cfl * int(round(8 / cfl))
     m0, m1 = U0[0, 0, 3, 3, 3:-3].sum(), U[0, 0, 3, 3, 3:-3].sum()
     assert abs((m1 - m0) - t_over_dx * (Dv[0] - Dv[1])) < 1e-10 * abs(m0)
+
+
+def test_copy_boundary_ghost_fill_is_the_nearest_interior_cell(oracle):
+    """Pin of fill_ghosts_box, bc = "copy" ("copy" boundaries; l.170 user-supplied outer boundary): after a
+    step every ghost cell of every primitive holds the bits of the interior cell with the CLAMPED index -- faces, edges and
+    corners -- on a 3-D block with an off-diagonal metric whose interior values are all distinct, so that clamping to n or
+    n - 2, or treating an edge / corner direction by direction in the wrong way, fails.  Then the whole loop against the
+    independently written numpy loop of tests/evolve.py (its own clamp, ghost fill after every stage) over three SSP-RK2
+    steps: the fill happens where the method needs it."""
+    from evolve import fill_copy_bc, rk2_evolve
+    g = 3
+    prob = inputs.general_metric_box(n=(9, 7, 6), seed=11)
+    start = fill_copy_bc(prob.prim.copy(), g)
+    dt = 0.2 * min(prob.dx)
+    prim, U, nfail = oracle.evolve(start, prob.metric, prob.K, prob.dx, g, "minmod", prob.gamma, dt, 1, rk=2, bc="copy")
+    assert nfail == 0
+    inner = prim[prob.interior]
+    assert len(np.unique(inner[0, 0])) == inner[0, 0].size          # distinct values: a wrong source index is visible
+    Nz, Ny, Nx = prim.shape[2:]
+    kk, jj, ii = (np.clip(np.arange(N), g, N - g - 1) for N in (Nz, Ny, Nx))
+    want = prim[:, :, kk[:, None, None], jj[None, :, None], ii[None, None, :]]
+    assert np.array_equal(prim, want)
+    assert not np.array_equal(prim, start)                           # the step did change the block
+
+    class Backend:
+        def rhs(self, p):
+            return oracle.valencia_rhs(p, prob.metric, prob.K, prob.dx, g, "minmod", prob.gamma)[0]
+
+        def prim2con(self, p):
+            return oracle.prim2con(p, prob.metric, g, prob.gamma)
+
+        def con2prim(self, U):
+            return oracle.con2prim(U, prob.metric, g, prob.gamma)[0]
+
+    p_loop, U_loop = rk2_evolve(Backend(), start, g, dt, 3)
+    p_orc, U_orc, nfail = oracle.evolve(start, prob.metric, prob.K, prob.dx, g, "minmod", prob.gamma, dt, 3, rk=2, bc="copy")
+    assert nfail == 0
+    ii3 = prob.interior
+    assert np.abs(U_orc[ii3] - U_loop[ii3]).max() <= 1e-12 * np.abs(U_loop[ii3]).max()
+    assert np.abs(p_orc - p_loop).max() <= 1e-12 * np.abs(p_loop).max()     # ghosts included
