@@ -128,6 +128,14 @@ def test_ct_parity_config5_128_full_block(grx, oracle):
         _check(prob, recon, got, plain, fb, oracle, check_fb=False)
 
 
+def test_ct_parity_bench_workload_256_full_block(grx, oracle):
+    """The block bench.py times the CT entry point on (C5 256^3 x 1, WENO5; 296 CTAs in two waves, one z chunk of 256
+    planes per CTA, plus the rim face kernel and the curl kernel): every interior cell against the oracle."""
+    prob = inputs.sweep_boxes(256, 1)
+    got, plain, fb = _run(grx, prob, "weno5", "auto")
+    _check(prob, "weno5", got, plain, fb, oracle, check_fb=False)
+
+
 def test_ct_invalid_arguments(grx):
     import torch
     prob = inputs.general_metric_box(n=(8, 6, 5), seed=1)

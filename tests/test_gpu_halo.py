@@ -82,7 +82,11 @@ def test_one_slab_ring_equals_step_rk_periodic(grx, overlap):
     assert float((consA[ii] - grx.prim2con(prim, met, g, gamma)[ii]).abs().max()) > 1e-6      # it did move
 
 
-def test_two_slab_ring_in_one_process_equals_the_undivided_domain(grx):
+@pytest.mark.parametrize("transport", ["pull", "pack"])
+def test_two_slab_ring_in_one_process_equals_the_undivided_domain(grx, oracle, transport):
+    """Two z slabs exchanging ghost planes (peer-memory pull kernel, or pack / copy / unpack) against (a) grx_step_rk on the
+    undivided periodic domain, bit for bit, and (b) the oracle's method-of-lines loop on the undivided domain
+    (oracle_evolve, periodic ghosts filled here with numpy), 1e-10 max|U| per component."""
     import torch
     from paper_2210_17509_b200 import halo
     g = inputs.NGHOST
@@ -90,8 +94,12 @@ def test_two_slab_ring_in_one_process_equals_the_undivided_domain(grx):
     prim_h, met_h, K_h, dx, gamma = _periodic_problem((18, 10, 2 * nz), 9)
     met_h = np.ascontiguousarray(np.broadcast_to(met_h[:, :, 6:7], met_h.shape))
     K_h = np.ascontiguousarray(np.broadcast_to(K_h[:, :, 6:7], K_h.shape))
+    # periodic ghosts on the host (no library call on the oracle's input)
+    prim_h = np.ascontiguousarray(np.pad(prim_h[:, :, g:-g, g:-g, g:-g], ((0, 0), (0, 0), (g, g), (g, g), (g, g)), mode="wrap"))
     prim, met, K = _dev(prim_h, met_h, K_h)
-    grx.fill_ghosts(prim, g, "periodic", 7)
+    filled = prim.clone()
+    grx.fill_ghosts(filled, g, "periodic", 7)
+    assert torch.equal(filled, prim)            # the library's periodic fill is this wrap
     dt = 0.2 * min(dx)
     cons = grx.prim2con(prim, met, g, gamma)
     whole_p = prim.clone()
@@ -103,7 +111,11 @@ def test_two_slab_ring_in_one_process_equals_the_undivided_domain(grx):
     for r in range(2):
         p, m, k = cut(prim, r), cut(met, r), cut(K, r)
         slabs.append(dict(prim=p, met=m, K=k, cons=grx.prim2con(p, m, g, gamma), U0=torch.empty_like(p), L=torch.empty_like(p)))
-    exs = [halo.ZSlabExchange(s["prim"], g) for s in slabs]
+    if transport == "pull":
+        exs = [halo.ZSlabExchange(s["prim"], g) for s in slabs]
+    else:   # the packing kernels, launched on the exchange's own stream (torch's current stream inside start / finish)
+        exs = [halo.ZSlabExchange(s["prim"], g, pack=lambda p, gg, side, buf: grx.halo_z(p, gg, side, False, buf),
+                                  unpack=lambda p, gg, side, buf: grx.halo_z(p, gg, side, True, buf)) for s in slabs]
     halo.ZSlabExchange.link_ring(exs)
 
     def rhs_all():
@@ -133,6 +145,13 @@ def test_two_slab_ring_in_one_process_equals_the_undivided_domain(grx):
         a = s["cons"][:, :, g:-g, g:-g, g:-g]
         b = cons[:, :, g + r * nz:g + (r + 1) * nz, g:-g, g:-g]
         assert torch.equal(a, b), f"slab {r}"
+    # against the oracle on the undivided domain
+    _, U_ref, nfail = oracle.evolve(prim_h, met_h, K_h, dx, g, "weno5", gamma, dt, 2, rk=2, bc="periodic")
+    assert nfail == 0
+    ring = np.concatenate([s["cons"][:, :, g:-g, g:-g, g:-g].cpu().numpy() for s in slabs], axis=2)
+    ref = U_ref[:, :, g:-g, g:-g, g:-g]
+    for c in range(8):
+        assert np.abs(ring[:, c] - ref[:, c]).max() <= 1e-10 * np.abs(ref[:, c]).max(), c
 
 
 def test_halo_pack_unpack_roundtrip(grx):

@@ -477,6 +477,57 @@ def test_device_resident_steps_vs_oracle_loop(grx, oracle, case):
     assert np.abs(prim.cpu().numpy() - p_ref).max() < 1e-9 * np.abs(p_ref).max()
 
 
+def test_device_resident_steps_config5_128_full_block(grx, oracle):
+    """grx_step_rk at a size of the sweep (C5 128^3 x 1, WENO5, SSP-RK2, copy boundaries): two steps against oracle_evolve on
+    every interior cell -- the multi-wave launch geometry of the right-hand side inside the stepping loop, the fused stage /
+    con2prim kernel and the ghost fill on a block of several hundred tiles."""
+    import torch
+    from evolve import fill_copy_bc
+    prob = inputs.sweep_boxes(128, 1)
+    g = prob.nghost
+    prim0 = fill_copy_bc(prob.prim.copy(), g)
+    dt = 0.2 * min(prob.dx)
+    p_ref, U_ref, nf_ref = oracle.evolve(prim0, prob.metric, prob.K, prob.dx, g, "weno5", prob.gamma, dt, 2, rk=2, bc="copy")
+    assert nf_ref == 0
+    prim = torch.from_numpy(prim0).cuda()
+    met, K = torch.from_numpy(prob.metric).cuda(), torch.from_numpy(prob.K).cuda()
+    cons = grx.prim2con(prim, met, g, prob.gamma)
+    nfail = torch.zeros(1, dtype=torch.int64, device="cuda")
+    grx.step_rk(cons, prim, met, K, prob.dx, g, "weno5", prob.gamma, dt, 2, rk=2, bc="copy", nfail=nfail)
+    torch.cuda.synchronize()
+    assert int(nfail.item()) == 0
+    ii = prob.interior
+    assert relerr_per_component(cons.cpu().numpy()[ii], U_ref[ii]).max() < 1e-10
+    assert np.abs(prim.cpu().numpy() - p_ref).max() < 1e-9 * np.abs(p_ref).max()
+
+
+@pytest.mark.parametrize("test,cfl", [(2, 0.8), (3, 0.4), (4, 0.2), (5, 0.8)])
+def test_device_resident_steps_balsara_2_to_5(grx, oracle, test, cfl):
+    """NEXT-1 "runs Balsara 1-5 end to end": the Table I states of Balsara 2-5 (minmod + HLLE + RK4,
+    copy boundaries l.255, 200 cells, the CFLs at which the oracle's bare loop survives, tests/test_oracle_evolve.py)
+    through grx_step_rk against oracle_evolve.  The 10^4 pressure jump of Balsara 3 and the W = 22 collision of Balsara 4 are
+    where the warm-started con2prim of the stage kernel has to fall back to its bracketed solve; it must converge in every
+    cell (nfail = 0) as the oracle's does."""
+    import torch
+    from test_oracle_evolve import shocktube
+    prob, _ = shocktube(test, 200)
+    g = prob.nghost
+    dt, nsteps = cfl * prob.dx[0], int(round(8 / cfl))
+    p_ref, U_ref, nf_ref = oracle.evolve(prob.prim, prob.metric, prob.K, prob.dx, g, "minmod", prob.gamma, dt, nsteps, rk=4,
+                                         bc="copy")
+    assert nf_ref == 0
+    prim = torch.from_numpy(prob.prim.copy()).cuda()
+    met, K = torch.from_numpy(prob.metric).cuda(), torch.from_numpy(prob.K).cuda()
+    cons = grx.prim2con(prim, met, g, prob.gamma)
+    nfail = torch.zeros(1, dtype=torch.int64, device="cuda")
+    grx.step_rk(cons, prim, met, K, prob.dx, g, "minmod", prob.gamma, dt, nsteps, rk=4, bc="copy", nfail=nfail)
+    torch.cuda.synchronize()
+    assert int(nfail.item()) == 0
+    ii = prob.interior
+    assert relerr_per_component(cons.cpu().numpy()[ii], U_ref[ii]).max() < 1e-10
+    assert np.abs(prim.cpu().numpy() - p_ref).max() < 1e-9 * np.abs(p_ref).max()
+
+
 def test_steps_with_constrained_transport_keep_the_vertex_divergence(grx):
     """grx_step_rk_ct on a periodic multi-tile block whose field is not solenoidal: the vertex-centred divergence of calB
     after 5 RK2 steps is the initial one to rounding; without CT it is not."""

@@ -73,6 +73,29 @@ def test_vertex_rhs_parity(grx, oracle, n, nbox, variant):
         assert int(cnt.item()) == nfb_ref
 
 
+def test_vertex_rhs_parity_256_full_block(grx, oracle):
+    """The size bench.py times grx_valencia_rhs_vertex at (256^3 interior, 257^3-vertex metric, WENO5): every interior cell
+    against the oracle, fallback count included."""
+    import torch
+    prim, met_v, K_v, dx = _vertex_problem((256, 256, 256))
+    gamma = 5.0 / 3.0
+    ref, nfb_ref = oracle.valencia_rhs_vertex(prim, met_v, K_v, dx, G, "weno5", gamma)
+    d = _dev(prim, met_v, K_v)
+    out = torch.full_like(d[0], -7.25e300)
+    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    grx.set_fallback_counter(cnt)
+    try:
+        grx.valencia_rhs_vertex(*d, dx, G, "weno5", gamma, out=out)
+        torch.cuda.synchronize()
+    finally:
+        grx.set_fallback_counter(None)
+    got = out.cpu().numpy()
+    ii = (slice(None), slice(None), slice(G, -G), slice(G, -G), slice(G, -G))
+    rel = relerr_per_component(got[ii], ref[ii])
+    assert np.all(np.isfinite(got[ii])) and rel.max() <= TOL, rel
+    assert int(cnt.item()) == nfb_ref
+
+
 def test_vertex_rhs_linear_metric_equals_cell_centred_kernel(grx):
     """Pin V1 on the GPU: on a metric linear in the coordinates the vertex kernel reproduces the product (cell-centred)
     kernel to rounding."""
