@@ -61,6 +61,7 @@ NCU_CAPTURE = {
 KERNEL_OF_VARIANT = {"auto": "rhs_tma_kernel (rhs_fused_kernel for odd Nx)", "tma": "rhs_tma_kernel", "ldg": "rhs_fused_kernel",
                      "simple": "rhs_simple_kernel"}
 SWEEP_POINTS = ("c5-32", "c5-64", "c5-128", "c5-256", "c3", "c4")
+ORACLE_TIMED_POINTS = ("c5-64", "c5-128")     # sweep points at which the oracle is timed beside the kernel
 
 
 KERNEL_SOURCES = ("grx_tma.cu", "grx_math.cuh", "grx_common.cuh")   # what the kernel of a step is compiled from
@@ -80,6 +81,13 @@ def csrc_sha():
 def algorithmic_flops_per_cell(n, recon):
     a, b = FLOPS_MODEL[recon]
     return a + (b / 3.0) * (1.0 / n[0] + 1.0 / n[1] + 1.0 / n[2])
+
+
+def redundant_flops_per_cell(n):
+    """Operations the oracle's count holds twice: v_i and v^2 of the admissibility test (20 per face side, piece
+    `admissible` of tests/test_bench_model.py) are evaluated again inside prim2con_point.  Two sides of 3 + sum 1/n_d faces
+    per cell: 120 per cell of a large block.  `frac_no_redundancy` leaves them out of the numerator."""
+    return 20.0 * 2.0 * (3.0 + 1.0 / n[0] + 1.0 / n[1] + 1.0 / n[2])
 
 
 def algorithmic_bytes_per_cell(n, g):
@@ -190,6 +198,13 @@ def time_oracle(prob, recon, budget_s, reps=1):
     return cells / best, best, n1, orc.num_threads()
 
 
+def config_of(prob, recon, n_ranks):
+    """`config` of the JSON line, the same object in both arms (what differs between the arms is in `arm` / `variant`)."""
+    return {"workload": workload_string(prob, recon),
+            "l2": "GPU arm: inputs 4.6 GB >> 126 MB L2, no flush; reference arm: host caches, not flushed",
+            "parallelism": f"blocks x{n_ranks}, no collective (reference arm: rank 0's host cores)"}
+
+
 def workload_string(prob, recon):
     """The same text in both arms, so that the driver sees one config."""
     return (f"{prob.name} per GPU, {recon}+HLLE, Gamma-law EOS, perturbed conformally flat metric + shift + K_ij, "
@@ -227,7 +242,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_string(prob, args.recon), "l2": "n/a (CPU)", "arm": "oracle on host cores, bounded sample"},
+        "config": config_of(prob, args.recon, args.gpus), "arm": "oracle on host cores, bounded sample", "variant": "n/a",
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -269,19 +284,33 @@ def load_workload(name, rank, nbox=None):
     return inputs.by_name(name)
 
 
-def time_rhs(grx, torch, prob, dev, recon, steps, warmup, stream):
+def time_rhs(grx, torch, prob, dev, recon, steps, warmup, stream, per_call=None):
+    """`steps` calls between one pair of CUDA events on the launching stream (the returned total, what `value` and
+    `ms_per_step` come from); an event between consecutive calls as well, so that the median and the best single call can
+    be reported beside the mean: per_call, if a list, receives the milliseconds of every call."""
     prim, met, K = dev
     out = torch.empty_like(prim)
     for _ in range(warmup):
         grx.valencia_rhs(prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, out=out, stream=stream)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
     stream.synchronize()
-    e0.record(stream)
-    for _ in range(steps):
+    ev[0].record(stream)
+    for i in range(steps):
         grx.valencia_rhs(prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, out=out, stream=stream)
-    e1.record(stream)
+        ev[i + 1].record(stream)
     stream.synchronize()
-    return e0.elapsed_time(e1) * 1e-3, out
+    if per_call is not None:
+        per_call.extend(ev[i].elapsed_time(ev[i + 1]) for i in range(steps))
+    return ev[0].elapsed_time(ev[steps]) * 1e-3, out
+
+
+def call_stats(per_call):
+    """Median and best of the per-call milliseconds (the mean is ms_per_step)."""
+    if not per_call:
+        return {}
+    a = sorted(per_call)
+    n = len(a)
+    return {"ms_median": a[n // 2] if n % 2 else 0.5 * (a[n // 2 - 1] + a[n // 2]), "ms_best": a[0]}
 
 
 def time_zone_cycles(grx, torch, prob, dev, recon, stream, nsteps=5, ct=False):
@@ -407,37 +436,65 @@ def time_vertex(grx, torch, prob, dev, recon, stream, steps=5):
     return res
 
 
-def measure_dfma_peak(grx, torch, stream):
+class Probe:
+    """libgrx_probe.so (csrc/probe/grx_probe.h): the FP64 micro-benchmarks.  Bench-side code, not the product library."""
+
+    def __init__(self):
+        import ctypes as C
+        from paper_2210_17509_b200 import build
+        self.C = C
+        self.lib = C.CDLL(build.build_probe())
+        self.lib.grx_probe_dfma_peak.argtypes = [C.c_int, C.c_void_p, C.POINTER(C.c_double), C.c_void_p]
+        self.lib.grx_probe_fp64_issue.argtypes = [C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_double), C.c_void_p]
+
+    def _call(self, fn, *args, sink, stream):
+        n = self.C.c_double(0.0)
+        rc = fn(*args, self.C.c_void_p(sink.data_ptr()), self.C.byref(n), self.C.c_void_p(stream.cuda_stream))
+        if rc != 0:
+            raise RuntimeError(f"libgrx_probe: CUDA error {rc}")
+        return n.value
+
+    def dfma_peak(self, iters, sink, stream):
+        return self._call(self.lib.grx_probe_dfma_peak, iters, sink=sink, stream=stream)
+
+    def fp64_issue(self, mode, iters, sink, stream):
+        return self._call(self.lib.grx_probe_fp64_issue, mode, iters, sink=sink, stream=stream)
+
+
+def measure_dfma_peak(probe, torch, stream):
     sink = torch.zeros(1, dtype=torch.float64, device="cuda")
-    grx.dfma_peak_launch(2000, sink, stream)
+    probe.dfma_peak(2000, sink, stream)
     best = 0.0
     for _ in range(5):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        flops = grx.dfma_peak_launch(20000, sink, stream)
+        flops = probe.dfma_peak(20000, sink, stream)
         e1.record(stream)
         stream.synchronize()
         best = max(best, flops / (e0.elapsed_time(e1) * 1e-3))
     return best / 1e12
 
 
-ISSUE_PROBE_MODES = ("dfma_fixed_operands", "dfma_three_registers", "dmul", "dmul+imad", "dmul+sts64", "dmul+shfl")
+ISSUE_PROBE_MODES = ("dfma_fixed_operands", "dfma_three_registers", "dmul", "dmul+imad", "dmul+sts64", "dmul+shfl",
+                     "dfma_three_registers_mixed_parity", "dfma_accumulate_in_place", "dfma_operand_shared_by_two",
+                     "dfma_two_registers+constant")
 
 
-def measure_issue_probe(grx, torch, stream, sm_mhz):
-    """FP64 lanes per clock per SM (64 = nominal) of the issue probe's six patterns (include/grx.h): what an FP64
-    instruction costs with three register operands, and next to integer, store and shuffle instructions."""
+def measure_issue_probe(probe, torch, stream, sm_mhz):
+    """FP64 lanes per clock per SM (64 = nominal) of the issue probe's patterns (csrc/probe/grx_probe.h): what an FP64
+    instruction costs with three register operands (in several placements), and next to integer, store and shuffle
+    instructions."""
     sink = torch.zeros(1, dtype=torch.float64, device="cuda")
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     hz = (sm_mhz or 1965.0) * 1e6
     res = {}
     for mode, name in enumerate(ISSUE_PROBE_MODES):
-        grx.fp64_issue_probe(mode, 500, sink, stream)
+        probe.fp64_issue(mode, 500, sink, stream)
         best = 0.0
         for _ in range(3):
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(stream)
-            n = grx.fp64_issue_probe(mode, 4000, sink, stream)
+            n = probe.fp64_issue(mode, 4000, sink, stream)
             e1.record(stream)
             stream.synchronize()
             best = max(best, n / (e0.elapsed_time(e1) * 1e-3))
@@ -460,6 +517,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if rank == 0:
         build.build()
+        build.build_probe()
     if world > 1:
         dist.barrier()
     grx.lib()
@@ -487,7 +545,8 @@ def run_ours(args):
     time_rhs(grx, torch, prob, dev, recon, 0, max(args.warmup, 3), stream)
     barrier()
     with ClockSampler(local) as cs:
-        t_dev, out = time_rhs(grx, torch, prob, dev, recon, args.steps, 0, stream)
+        per_call = []
+        t_dev, out = time_rhs(grx, torch, prob, dev, recon, args.steps, 0, stream, per_call)
         barrier()
     clocks = cs.summary()
     if clocks["samples"] < 5:
@@ -539,12 +598,15 @@ def run_ours(args):
     by_cell = algorithmic_bytes_per_cell(prob.n, g)
     ach_tflops = fl_cell * cells / t_launch / 1e12
     ach_gbs = by_cell * cells / t_launch / 1e9
-    dfma = measure_dfma_peak(grx, torch, stream)
+    probe = Probe()
+    dfma = measure_dfma_peak(probe, torch, stream)
     roofline = {
         "bound": "alu", "kernel": KERNEL_OF_VARIANT[args.variant], "achieved": ach_tflops, "peak": FP64_PEAK_NOMINAL_TFLOPS,
         "unit": "TFLOP/s", "frac": ach_tflops / FP64_PEAK_NOMINAL_TFLOPS,
         "peak_source": "nominal FP64: 148 SM x 64 lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry)",
         "peak_dfma_measured": dfma, "frac_of_dfma_measured": ach_tflops / dfma if dfma > 0 else None,
+        "frac_no_redundancy": (fl_cell - redundant_flops_per_cell(prob.n)) * cells / t_launch / 1e12 / FP64_PEAK_NOMINAL_TFLOPS,
+        "redundant_flops_per_cell": redundant_flops_per_cell(prob.n),
         "flops_per_cell": fl_cell, "flops_source": "operations of the oracle's counting instance, pinned piece by piece "
                                                    "against hand counts (tests/test_bench_model.py)",
         "frac_survey_count": (FLOPS_SURVEY[recon] * cells / t_launch / 1e12 / FP64_PEAK_NOMINAL_TFLOPS
@@ -554,7 +616,7 @@ def run_ours(args):
         "hbm": {"achieved": ach_gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s", "peak_source": peak_src,
                 "frac": ach_gbs / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None},
         "traffic": None,
-        "fp64_lanes_per_clk_per_sm": measure_issue_probe(grx, torch, stream, clocks.get("sm_mhz")),
+        "fp64_lanes_per_clk_per_sm": measure_issue_probe(probe, torch, stream, clocks.get("sm_mhz")),
     }
     # profiler-only numbers: reported only for the state of the kernel sources they were captured at
     sha = csrc_sha()
@@ -591,11 +653,9 @@ def run_ours(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_string(prob, recon), "arm": "one grx_valencia_rhs call per step",
-                   "l2": "inputs 4.6 GB >> 126 MB L2, no flush", "variant": args.variant,
-                   "parallelism": f"blocks x{world}, no collective"},
+        "ms_per_step": 1e3 * t_max / args.steps, **call_stats(per_call), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_of(prob, recon, world), "arm": "one grx_valencia_rhs call per step", "variant": args.variant,
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "matches_device_path": e2e_ok},
@@ -633,15 +693,22 @@ def sweep_points(grx, torch, stream, names, steps, warmup, peaks, keep=None):
             dev = tuple(torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (prob.prim, prob.metric, prob.K))
             own = True
         for recon in prob.recons:
-            t, _ = time_rhs(grx, torch, prob, dev, recon, steps, max(warmup, 3), stream)
+            calls = []
+            t, _ = time_rhs(grx, torch, prob, dev, recon, steps, max(warmup, 3), stream, calls)
             tl = t / steps
             fl = algorithmic_flops_per_cell(prob.n, recon) * prob.cells / tl / 1e12
             gb = algorithmic_bytes_per_cell(prob.n, prob.nghost) * prob.cells / tl / 1e9
             pt = {"workload": prob.name, "recon": recon, "cells": prob.cells, "ms_per_call": 1e3 * tl,
                   "cell_updates_per_s": prob.cells / tl, "frac": fl / FP64_PEAK_NOMINAL_TFLOPS,
                   "hbm_frac": gb / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None}
+            pt.update(call_stats(calls))
             if recon in FLOPS_SURVEY:
                 pt["frac_survey_count"] = FLOPS_SURVEY[recon] * prob.cells / tl / 1e12 / FP64_PEAK_NOMINAL_TFLOPS
+            if name in ORACLE_TIMED_POINTS:
+                # the oracle is timed at these sizes too (bounded sample of box 0, 2 s)
+                rate, secs, n1, cores = time_oracle(prob, recon, budget_s=2.0)
+                pt["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                      "sample": f"first {n1[0]}x{n1[1]}x{n1[2]} interior cells of box 0, one evaluation, {secs:.1f} s"}
             pts.append(pt)
         if own:
             del dev, prob

@@ -263,30 +263,19 @@ int grx_step_rk_ct(const grx_grid* grid, double* cons, double* prim, const doubl
  * first-order fallback.  NULL switches counting off (the default; counting costs a few atomics). */
 int grx_debug_set_fallback_counter(unsigned long long* counter);
 
-/* Selects the kernel used by later grx_valencia_rhs calls of this PROCESS (default GRX_VARIANT_AUTO).  The path
- * SURVEY.md section 8(b) sketches for the R5 count, grx_debug_fallback_count(host_out, stream), is provided here as
- * grx_debug_set_fallback_counter above: a caller-owned device counter, so that counting stays asynchronous. */
+/* Debug (the call SURVEY.md section 8(b) sketches for the R5 count): copies the counter registered by this host thread
+ * with grx_debug_set_fallback_counter to *host_out (HOST pointer), ordered after the work already enqueued on `cuda_stream`,
+ * and synchronises that stream.  The value is what has accumulated since the caller last zeroed the counter: zero it
+ * before the call whose fallbacks are wanted to get "the count of the last call".  GRX_ERR_INVALID_ARG if host_out is NULL
+ * or no counter is registered on this thread; GRX_ERR_CUDA if the copy fails. */
+int grx_debug_fallback_count(unsigned long long* host_out, void* cuda_stream);
+
+/* Selects the kernel used by later grx_valencia_rhs calls of this PROCESS (default GRX_VARIANT_AUTO). */
 int grx_set_variant(int variant);
 
 /* Accuracy self-test of the division-free reciprocal / rsqrt / sqrt helpers the kernels use:
  * y[0..n) = 1/x, y[n..2n) = 1/sqrt(x), y[2n..3n) = sqrt(x) for x[0..n) > 0 (DEVICE pointers). */
 int grx_selftest_math(const double* x, double* y, size_t n, void* cuda_stream);
-
-/* Throughput of a dependent-chain-free DFMA loop on the whole device: launches the micro-benchmark
- * kernel once (iters FMAs per chain, 8 chains per thread, one resident wave) and writes a checksum to
- * `sink` (DEVICE pointer to one double).  flops_out (HOST) receives the flop count of that launch; time
- * it with CUDA events on `cuda_stream` to obtain the FP64 peak used as the roofline denominator. */
-int grx_dfma_peak_launch(int iters, double* sink, double* flops_out, void* cuda_stream);
-
-/* Issue probe behind the roofline discussion: one launch of a dependency-free FP64 loop over the
- * whole device (4 warps per scheduler, 16 independent values per thread) in one of six operand / neighbour patterns:
- *   0  a = fma(a, m, c), m and c fixed        1  fma of three distinct changing registers        2  mul of two registers
- *   3  pattern 2 + one independent IMAD per mul     4  pattern 2 + one STS.64 per mul     5  pattern 2 + one SHFL per mul
- * sink: DEVICE pointer to one double (checksum).  fp64_instr_out (HOST): FP64 thread-instructions of the launch; divide by
- * the event time, the SM count and the clock to get FP64 lanes per clock per SM (64 = the nominal peak).  Measured on
- * B200: 62 / 42 / 62 / 40 / 62 / 31 -- a DFMA with three register operands occupies the pipe for 3 cycles instead of 2,
- * and an integer or shuffle instruction between two FP64 instructions costs an FP64 issue slot (a store does not). */
-int grx_fp64_issue_probe(int mode, int iters, double* sink, double* fp64_instr_out, void* cuda_stream);
 
 /* Thread-local description of the last non-OK return of this thread ("" if none). */
 const char* grx_last_error(void);

@@ -16,6 +16,9 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgrx.so")
 OBJDIR = os.path.join(ROOT, "build", "grx")
 SOURCES = ["grx_api.cu", "grx_simple.cu", "grx_fused.cu", "grx_tma.cu", "grx_ct.cu", "grx_vertex.cu", "grx_support.cu"]
+# bench-side measurement probes: their own library, loaded by bench.py only (not part of the product ABI)
+PROBE_LIB = os.path.join(HERE, "libgrx_probe.so")
+PROBE_SRC = os.path.join(CSRC, "probe", "grx_probe.cu")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--fmad=true",
@@ -58,5 +61,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_probe(force: bool = False) -> str:
+    """csrc/probe/grx_probe.cu -> libgrx_probe.so (the FP64 micro-benchmarks of bench.py)."""
+    hdr = os.path.join(CSRC, "probe", "grx_probe.h")
+    if force or not os.path.exists(PROBE_LIB) or os.path.getmtime(PROBE_LIB) < max(os.path.getmtime(PROBE_SRC),
+                                                                                   os.path.getmtime(hdr)):
+        cmd = [NVCC, *ARCH, "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-shared", "-o", PROBE_LIB, PROBE_SRC,
+               "-cudart", "static"]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("nvcc failed for grx_probe.cu:\n%s\n%s" % (r.stdout, r.stderr))
+    return PROBE_LIB
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build_probe(force="--force" in sys.argv))

@@ -679,6 +679,17 @@ int grx_debug_set_fallback_counter(unsigned long long* counter) {
     return GRX_OK;
 }
 
+int grx_debug_fallback_count(unsigned long long* host_out, void* cuda_stream) {
+    if (!host_out) return fail(GRX_ERR_INVALID_ARG, "host_out is NULL");
+    if (!t_fallback_counter)
+        return fail(GRX_ERR_INVALID_ARG, "no fallback counter registered on this thread (grx_debug_set_fallback_counter)");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    cudaError_t e = cudaMemcpyAsync(host_out, t_fallback_counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail_cuda(e, "grx_debug_fallback_count");
+    return GRX_OK;
+}
+
 int grx_set_variant(int variant) {
     if (variant != GRX_VARIANT_AUTO && variant != GRX_VARIANT_SIMPLE && variant != GRX_VARIANT_LDG && variant != GRX_VARIANT_TMA)
         return fail(GRX_ERR_INVALID_ARG, "unknown variant");
@@ -690,20 +701,6 @@ int grx_selftest_math(const double* x, double* y, size_t n, void* cuda_stream) {
     if (n && (!x || !y)) return fail(GRX_ERR_INVALID_ARG, "NULL array pointer");
     const cudaError_t e = grx::launch_selftest_math(x, y, n, static_cast<cudaStream_t>(cuda_stream));
     if (e != cudaSuccess) return fail_cuda(e, "grx_selftest_math launch");
-    return GRX_OK;
-}
-
-int grx_dfma_peak_launch(int iters, double* sink, double* flops_out, void* cuda_stream) {
-    if (iters < 1 || !sink) return fail(GRX_ERR_INVALID_ARG, "iters must be >= 1 and sink non-NULL");
-    const cudaError_t e = grx::launch_dfma_peak(iters, sink, flops_out, static_cast<cudaStream_t>(cuda_stream));
-    if (e != cudaSuccess) return fail_cuda(e, "grx_dfma_peak_launch");
-    return GRX_OK;
-}
-
-int grx_fp64_issue_probe(int mode, int iters, double* sink, double* fp64_instr_out, void* cuda_stream) {
-    if (mode < 0 || mode > 5 || iters < 1 || !sink) return fail(GRX_ERR_INVALID_ARG, "mode must be 0..5, iters >= 1 and sink non-NULL");
-    const cudaError_t e = grx::launch_issue_probe(mode, iters, sink, fp64_instr_out, static_cast<cudaStream_t>(cuda_stream));
-    if (e != cudaSuccess) return fail_cuda(e, "grx_fp64_issue_probe");
     return GRX_OK;
 }
 

@@ -76,7 +76,5 @@ cudaError_t launch_fill_ghosts(const RhsParams& geom, double* prim, int bc, int 
 cudaError_t launch_halo_z(const RhsParams& geom, double* prim, double* buf, int side, bool unpack, cudaStream_t st);
 cudaError_t launch_halo_z_pull(const RhsParams& geom, double* prim, const double* below, const double* above, cudaStream_t st);
 cudaError_t launch_selftest_math(const double* x, double* y, size_t n, cudaStream_t st);
-cudaError_t launch_dfma_peak(int iters, double* sink, double* flops_out, cudaStream_t st);
-cudaError_t launch_issue_probe(int mode, int iters, double* sink, double* fp64_instr_out, cudaStream_t st);
 
 }  // namespace grx

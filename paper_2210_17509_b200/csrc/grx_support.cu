@@ -159,27 +159,6 @@ __global__ void selftest_math_kernel(const double* __restrict__ x, double* __res
     y[2 * n + t] = sqrt_nn(v);
 }
 
-// 8 independent FMA chains per thread; every lane of the FP64 pipe busy, nothing else going on.
-constexpr int DFMA_CHAINS = 8;
-constexpr int DFMA_THREADS = 256;
-__global__ void __launch_bounds__(DFMA_THREADS) dfma_peak_kernel(int iters, double* sink) {
-    double a[DFMA_CHAINS];
-    const double m = 1.0 + 1e-9 * threadIdx.x, c = 1e-12 * blockIdx.x;
-#pragma unroll
-    for (int q = 0; q < DFMA_CHAINS; ++q) a[q] = 0.1 * (q + 1);
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-#pragma unroll
-            for (int q = 0; q < DFMA_CHAINS; ++q) a[q] = fma(a[q], m, c);
-        }
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int q = 0; q < DFMA_CHAINS; ++q) s += a[q];
-    if (s == 1.2345678) *sink = s;   // keeps the chains alive without a store in the common case
-}
-
 cudaError_t launch_prim2con(const double* prim, const double* met, long long nc, int nbox, double gamma, double* cons,
                             cudaStream_t st) {
     const dim3 grid((unsigned)((nc + 255) / 256), nbox);
@@ -234,75 +213,6 @@ cudaError_t launch_halo_z_pull(const RhsParams& p, double* prim, const double* b
 cudaError_t launch_selftest_math(const double* x, double* y, size_t n, cudaStream_t st) {
     if (n == 0) return cudaSuccess;
     selftest_math_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(x, y, n);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_dfma_peak(int iters, double* sink, double* flops_out, cudaStream_t st) {
-    int dev = 0, sms = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (e != cudaSuccess) return e;
-    const int blocks = sms * 4;   // 4 x 256 threads per SM: 8 warps per scheduler
-    dfma_peak_kernel<<<blocks, DFMA_THREADS, 0, st>>>(iters, sink);
-    if (flops_out) *flops_out = 2.0 * 4.0 * DFMA_CHAINS * (double)iters * DFMA_THREADS * (double)blocks;
-    return cudaGetLastError();
-}
-
-// ---- issue probe: what an FP64 instruction really costs next to its operands and its neighbours ---------------
-// 16 independent values per thread, every instruction reads values written 9 or more instructions earlier, so
-// neither latency nor the reuse cache limits the rate.  MODE 0: a = fma(a, m, c) with m, c fixed (the classic peak loop);
-// 1: DFMA with three distinct, changing register operands; 2: DMUL of two registers; 3: 2 + one independent IMAD per
-// DMUL; 4: 2 + one STS.64 per DMUL; 5: 2 + one SHFL per DMUL.
-constexpr int PROBE_THREADS = 256, PROBE_VALUES = 16;
-template <int MODE>
-__global__ void __launch_bounds__(PROBE_THREADS) issue_probe_kernel(int iters, double* sink) {
-    __shared__ double sh[PROBE_THREADS * 8];
-    double r[PROBE_VALUES];
-    int x[8];
-    const double m = 1.0 - 1e-9 * (threadIdx.x & 7), c = 1e-12 * blockIdx.x;
-#pragma unroll
-    for (int i = 0; i < PROBE_VALUES; ++i) r[i] = 1.0 + 1e-9 * (threadIdx.x + i);
-#pragma unroll
-    for (int i = 0; i < 8; ++i) { x[i] = threadIdx.x + i; sh[threadIdx.x + PROBE_THREADS * i] = 1.0; }
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int i = 0; i < PROBE_VALUES; ++i) {
-            const int j = (i + 1) % PROBE_VALUES, l = (i + 7) % PROBE_VALUES, n = (i + 11) % PROBE_VALUES;
-            if (MODE == 0) r[i] = fma(r[i], m, c);
-            if (MODE == 1) r[i] = fma(r[j], r[l], r[n]);
-            if (MODE >= 2) r[i] = r[j] * r[l];
-            if (MODE == 3) x[i % 8] = x[i % 8] * 5 + x[(i + 3) % 8];
-            if (MODE == 4) sh[threadIdx.x + PROBE_THREADS * (i % 8)] = r[n];
-            if (MODE == 5) x[i % 8] = __shfl_xor_sync(0xffffffffu, x[i % 8], 1);
-        }
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int i = 0; i < PROBE_VALUES; ++i) s += r[i];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) s += x[i] + sh[(threadIdx.x * 7 + PROBE_THREADS * i) % (PROBE_THREADS * 8)];
-    if (s == 1.2345678) *sink = s;
-}
-
-cudaError_t launch_issue_probe(int mode, int iters, double* sink, double* fp64_instr_out, cudaStream_t st) {
-    int dev = 0, sms = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (e != cudaSuccess) return e;
-    const int blocks = sms * 2;   // 2 x 256 threads per SM: 4 warps per scheduler
-    switch (mode) {
-        case 0: issue_probe_kernel<0><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
-        case 1: issue_probe_kernel<1><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
-        case 2: issue_probe_kernel<2><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
-        case 3: issue_probe_kernel<3><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
-        case 4: issue_probe_kernel<4><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
-        case 5: issue_probe_kernel<5><<<blocks, PROBE_THREADS, 0, st>>>(iters, sink); break;
-        default: return cudaErrorInvalidValue;
-    }
-    // FP64 thread-instructions of the launch (one per value and iteration)
-    if (fp64_instr_out) *fp64_instr_out = (double)PROBE_VALUES * (double)iters * PROBE_THREADS * (double)blocks;
     return cudaGetLastError();
 }
 

@@ -20,8 +20,8 @@ EXPORTS = (
     "grx_valencia_rhs", "grx_valencia_rhs_host", "grx_host_workspace_bytes", "grx_prim2con", "grx_con2prim", "grx_rk_axpy",
     "grx_step_rk", "grx_step_workspace_bytes", "grx_step_rk_ct", "grx_step_ct_workspace_bytes", "grx_valencia_rhs_ct", "grx_ct_workspace_bytes",
     "grx_valencia_rhs_ct_static", "grx_ct_static_max_bytes",
-    "grx_valencia_rhs_vertex", "grx_tmunu_vertices", "grx_valencia_rhs_zrange", "grx_halo_z", "grx_halo_z_bytes", "grx_halo_z_pull", "grx_fill_ghosts", "grx_rk_stage", "grx_debug_set_fallback_counter",
-    "grx_set_variant", "grx_selftest_math", "grx_dfma_peak_launch", "grx_fp64_issue_probe", "grx_last_error", "grx_version",
+    "grx_valencia_rhs_vertex", "grx_tmunu_vertices", "grx_valencia_rhs_zrange", "grx_halo_z", "grx_halo_z_bytes", "grx_halo_z_pull", "grx_fill_ghosts", "grx_rk_stage", "grx_debug_set_fallback_counter", "grx_debug_fallback_count",
+    "grx_set_variant", "grx_selftest_math", "grx_last_error", "grx_version",
     "grx_weno_eps", "grx_v2max",
 )
 
@@ -71,10 +71,9 @@ def lib():
         L.grx_valencia_rhs_vertex.argtypes = [gp, vp, vp, vp, d3, i, i, dbl, vp, vp]
         L.grx_tmunu_vertices.argtypes = [gp, vp, vp, i, dbl, vp, vp]
         L.grx_debug_set_fallback_counter.argtypes = [vp]
+        L.grx_debug_fallback_count.argtypes = [C.POINTER(C.c_ulonglong), vp]
         L.grx_set_variant.argtypes = [i]
         L.grx_selftest_math.argtypes = [vp, vp, sz, vp]
-        L.grx_dfma_peak_launch.argtypes = [i, vp, d3, vp]
-        L.grx_fp64_issue_probe.argtypes = [i, i, vp, d3, vp]
         for name in EXPORTS:
             getattr(L, name).restype = C.c_int
         L.grx_host_workspace_bytes.restype = sz
@@ -362,6 +361,14 @@ def set_fallback_counter(counter):
     _check(lib().grx_debug_set_fallback_counter(C.c_void_p(counter.data_ptr()) if counter is not None else C.c_void_p(0)))
 
 
+def fallback_count(stream=None):
+    """grx_debug_fallback_count: value of the counter registered with set_fallback_counter, after the work enqueued on the
+    stream (synchronises it)."""
+    n = C.c_ulonglong(0)
+    _check(lib().grx_debug_fallback_count(C.byref(n), _stream(stream)))
+    return int(n.value)
+
+
 def set_variant(name):
     _check(lib().grx_set_variant(VARIANT[name] if isinstance(name, str) else int(name)))
 
@@ -373,21 +380,6 @@ def selftest_math(x):
     y = torch.empty(3 * n, dtype=torch.float64, device=x.device)
     _check(lib().grx_selftest_math(_dev(x), _dev(y), n, _stream()))
     return y[:n], y[n:2 * n], y[2 * n:]
-
-
-def dfma_peak_launch(iters, sink, stream=None):
-    """Launches the DFMA micro-benchmark once; returns the flop count of the launch."""
-    flops = C.c_double(0.0)
-    _check(lib().grx_dfma_peak_launch(int(iters), _dev(sink), C.byref(flops), _stream(stream)))
-    return flops.value
-
-
-def fp64_issue_probe(mode, iters, sink, stream=None):
-    """Launches the FP64 issue probe once in operand pattern `mode` (0..5, include/grx.h); returns the FP64
-    thread-instruction count of the launch."""
-    n = C.c_double(0.0)
-    _check(lib().grx_fp64_issue_probe(int(mode), int(iters), _dev(sink), C.byref(n), _stream(stream)))
-    return n.value
 
 
 def version():

@@ -61,6 +61,9 @@ def test_host_side_validation(lib):
         assert rc == 1, (why, rc)
         assert why in lib.grx_last_error().decode(), (why, lib.grx_last_error())
     assert lib.grx_prim2con(C.byref(g), None, fake, 3, 2.0, out, None) == 1
+    n = C.c_ulonglong(0)
+    assert lib.grx_debug_fallback_count(C.byref(n), None) == 1 and "no fallback counter" in lib.grx_last_error().decode()
+    assert lib.grx_debug_fallback_count(None, None) == 1
     assert lib.grx_set_variant(9) == 1
     assert lib.grx_set_variant(0) == 0
     assert lib.grx_host_workspace_bytes(C.byref(g), 3) == 32 * 14 ** 3 * 8

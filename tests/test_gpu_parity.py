@@ -42,6 +42,8 @@ def gpu_rhs(grx, prob, recon, variant="auto", count=False):
     try:
         grx.valencia_rhs(prim, met, K, prob.dx, prob.nghost, recon, prob.gamma, out=out)
         torch.cuda.synchronize()
+        if count:
+            assert grx.fallback_count() == int(cnt.item())      # grx_debug_fallback_count reads the same counter
     finally:
         grx.set_fallback_counter(None)
         grx.set_variant("auto")
