@@ -646,28 +646,30 @@ static int step_rk_impl(const grx_grid* grid, double* cons, double* prim, const 
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     cudaError_t e = cudaSuccess;
     auto rhs = [&]() { return ct ? launch_rhs_ct(p, recon, st, nullptr) : launch_variant(p, recon, st); };
-    auto stage = [&](double a, const double* Ua, double b, const double* Ub, double h, double* ac, double wdt) {
-        cudaError_t r = grx::launch_rk_stage(p, a, Ua, b, Ub, h, L, cons, ac, wdt, prim, nfail, st);
+    auto stage = [&](double a, const double* Ua, double b, const double* Ub, double h, double* Uout, double* ac, double wdt) {
+        cudaError_t r = grx::launch_rk_stage(p, a, Ua, b, Ub, h, L, Uout, ac, wdt, prim, nfail, st);
         return r != cudaSuccess ? r : grx::launch_fill_ghosts(p, prim, bc, 7, st);
     };
-    // L lives in the workspace: its ghost cells are never read or written
+    // `cons` keeps U^n until the last stage of a step overwrites it; the intermediate stage states go to the first
+    // workspace array (W) -- no copy of cons per step.  The next right-hand side reads prim only, so W is needed again
+    // only where a stage combines it (RK2).  L and W live in the workspace: their ghost cells are never read or written.
+    double* W = U0;
     for (int s = 0; s < nsteps && e == cudaSuccess; ++s) {
-        e = cudaMemcpyAsync(U0, cons, arr * sizeof(double), cudaMemcpyDeviceToDevice, st);
         if (rk_order == 2) {
+            e = rhs();
+            if (e == cudaSuccess) e = stage(0.0, cons, 1.0, cons, dt, W, nullptr, 0.0);      // U1 = U0 + dt L(P0)
             if (e == cudaSuccess) e = rhs();
-            if (e == cudaSuccess) e = stage(0.0, U0, 1.0, U0, dt, nullptr, 0.0);       // U1 = U0 + dt L(P0)
-            if (e == cudaSuccess) e = rhs();
-            if (e == cudaSuccess) e = stage(0.5, U0, 0.5, cons, dt, nullptr, 0.0);     // U = 1/2 U0 + 1/2 (U1 + dt L(P1))
+            if (e == cudaSuccess) e = stage(0.5, cons, 0.5, W, dt, cons, nullptr, 0.0);      // U = 1/2 U0 + 1/2 (U1 + dt L(P1))
         } else {
             const double w[4] = {1.0 / 6.0, 1.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0}, hs[3] = {0.5, 0.5, 1.0};
-            if (e == cudaSuccess) e = cudaMemcpyAsync(acc, cons, arr * sizeof(double), cudaMemcpyDeviceToDevice, st);
+            e = cudaMemcpyAsync(acc, cons, arr * sizeof(double), cudaMemcpyDeviceToDevice, st);
             for (int k = 0; k < 3 && e == cudaSuccess; ++k) {
                 e = rhs();
-                if (e == cudaSuccess) e = stage(0.0, U0, 1.0, U0, hs[k] * dt, acc, w[k] * dt);   // U = U0 + h dt k_k
+                if (e == cudaSuccess) e = stage(0.0, cons, 1.0, cons, hs[k] * dt, W, acc, w[k] * dt);   // U = U0 + h dt k_k
             }
             if (e == cudaSuccess) e = rhs();
             // the last weight goes in as the stage's own step: U = (U0 + dt/6 (k1 + 2 k2 + 2 k3)) + dt/6 k4
-            if (e == cudaSuccess) e = stage(0.0, U0, 1.0, acc, w[3] * dt, nullptr, 0.0);         // U = acc + dt/6 k4
+            if (e == cudaSuccess) e = stage(0.0, cons, 1.0, acc, w[3] * dt, cons, nullptr, 0.0);        // U = acc + dt/6 k4
         }
     }
     if (e != cudaSuccess) return fail_cuda(e, "grx_step_rk");

@@ -194,23 +194,23 @@ def step_rk2_zslabs(exch, cons, prim, metric, K, dx, nghost, recon, gamma, dt, n
     """`nsteps` SSP-RK2 steps (R21) of this rank's slab of a domain that is periodic in x, y (per rank) and z (over the
     ring): per stage  L = rhs_overlapped(prim);  U <- a U0 + b (U + dt L) fused with con2prim (grx_rk_stage);  x / y ghost
     fill (grx_fill_ghosts, dirs = 3).  `prim` must come with filled x / y ghosts; its z ghosts are exchanged here.
-    work: two arrays shaped like cons (U0 and L)."""
+    work: two arrays shaped like cons (U1 and L)."""
     from . import grx
     if stream is not None and cons.is_cuda:
         import torch
         if stream != torch.cuda.current_stream(cons.device):
-            # U0.copy_ below is a torch operation and goes to torch's current stream: make `stream` that stream
+            # any torch operation a caller's pack / unpack hooks issue goes to torch's current stream: make `stream` that one
             with torch.cuda.stream(stream):
                 return step_rk2_zslabs(exch, cons, prim, metric, K, dx, nghost, recon, gamma, dt, nsteps, work, overlap,
                                        nfail, stream)
-    U0, L = work
+    U1, L = work
     for _ in range(nsteps):
-        U0.copy_(cons)
+        # cons keeps U^n until the second stage overwrites it; U1 goes to the first work array (no copy of cons per step)
         rhs_overlapped(exch, prim, metric, K, dx, nghost, recon, gamma, L, overlap, stream)
-        grx.rk_stage(nghost, 0.0, U0, 1.0, U0, dt, L, cons, metric, gamma, prim, nfail=nfail, stream=stream)
+        grx.rk_stage(nghost, 0.0, cons, 1.0, cons, dt, L, U1, metric, gamma, prim, nfail=nfail, stream=stream)
         grx.fill_ghosts(prim, nghost, "periodic", 3, stream=stream)
         rhs_overlapped(exch, prim, metric, K, dx, nghost, recon, gamma, L, overlap, stream)
-        grx.rk_stage(nghost, 0.5, U0, 0.5, cons, dt, L, cons, metric, gamma, prim, nfail=nfail, stream=stream)
+        grx.rk_stage(nghost, 0.5, cons, 0.5, U1, dt, L, cons, metric, gamma, prim, nfail=nfail, stream=stream)
         grx.fill_ghosts(prim, nghost, "periodic", 3, stream=stream)
     # leave prim with consistent z ghosts
     exch.start(prim, stream)
