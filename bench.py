@@ -53,10 +53,10 @@ FLOPS_SURVEY = {"weno5": 4085.0, "minmod": 2140.0}
 # thread instructions per cell.  They belong to ONE state of the kernel sources: `csrc_sha` is the hash of
 # paper_2210_17509_b200/csrc/ they were captured at, and bench.py reports them only while the hash still matches.
 NCU_CAPTURE = {
-    "csrc_sha": "95efb3edba68",
-    "source": "profiles/r2_ncu_tma.md",
-    "c5-256/weno5/auto": {"traffic": 4.685476e9, "pipe_fp64_pct": 59.87, "fp64_inst_per_cell": 2750.0},
-    "c5-256/minmod/auto": {"traffic": 4.647681e9, "pipe_fp64_pct": 47.91, "fp64_inst_per_cell": 1509.0},
+    "csrc_sha": "d4fa1b786c4a",
+    "source": "profiles/r3_ncu_tma.md",
+    "c5-256/weno5/auto": {"traffic": 4.718020e9, "pipe_fp64_pct": 59.94, "fp64_inst_per_cell": 2750.0},
+    "c5-256/minmod/auto": {"traffic": 4.660311e9, "pipe_fp64_pct": 47.87, "fp64_inst_per_cell": 1509.0},
 }
 KERNEL_OF_VARIANT = {"auto": "rhs_tma_kernel (rhs_fused_kernel for odd Nx)", "tma": "rhs_tma_kernel", "ldg": "rhs_fused_kernel",
                      "simple": "rhs_simple_kernel"}
